@@ -1,0 +1,949 @@
+// mg_toroidal.cu -- C-ABI library (include/mg_toroidal.h): handle, setup, V-cycle, coarse GMRES, FGMRES.
+// Host code only orchestrates; every step of the path runs in the kernels of kernels_*.cuh.
+#include "../../include/mg_toroidal.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "kernels_bsr.cuh"
+#include "kernels_setup.cuh"
+#include "kernels_vec.cuh"
+
+using namespace mgk;
+
+namespace {
+
+thread_local std::string g_last_cuda_error;
+
+struct Level {
+    int n_phi = 0;
+    int64_t n_brows = 0, nnzb = 0, nvec = 0;
+    const int64_t *row_ptr = nullptr;
+    const int32_t *col_idx = nullptr;
+    const double *vals = nullptr;
+    int64_t *diag_pos = nullptr;
+    double *dinv = nullptr;
+    double rho_est = 0.0, lam_min = 0.0, lam_max = 0.0;
+    double *x = nullptr, *r = nullptr, *d[2] = {nullptr, nullptr}, *pe = nullptr, *rhs = nullptr;
+    std::vector<int64_t> h_row_ptr;  // host copies of the pattern (Galerkin symbolic phase)
+    std::vector<int32_t> h_col_idx;
+};
+
+struct Gmres {
+    GmresDev dev{};
+    int m = 0, maxit = 0;
+    int64_t n = 0, stride = 0;
+    double *V = nullptr, *Z = nullptr;
+    double *partial = nullptr;
+    unsigned *counter = nullptr;
+    int red_grid = 0;
+    bool flexible = false;
+    bool ready = false;
+};
+
+}  // namespace
+
+struct mg_handle {
+    mg_options opt{};
+    int b = 0, n_pol = 0, n_phi = 0, n_levels = 0;
+    cudaStream_t stream = nullptr;      // active stream: the caller's, or cap_stream while a graph is captured
+    cudaStream_t cap_stream = nullptr;  // internal non-default stream (the legacy default stream cannot capture)
+    std::vector<Level> lev;
+    std::vector<void *> owned;
+    int64_t dev_bytes = 0;
+    int64_t launches = 0;
+    int *pinned = nullptr;        // 8 ints + 4 doubles of pinned host scratch
+    double *pinned_d = nullptr;
+    // scratch reduction (power iteration, norms)
+    double *red_partial = nullptr, *red_out = nullptr;
+    unsigned *red_counter = nullptr;
+    Gmres coarse, outer;
+    cudaGraphExec_t coarse_graph = nullptr;
+    int64_t coarse_graph_kernels = 0;
+    bool capturing = false;
+    int64_t capture_count = 0;
+    double *d_rhs_host = nullptr, *d_x_host = nullptr;  // device staging for mg_solve_host
+    int coarse_iters_total = 0, coarse_iters_last = 0;
+};
+
+namespace {
+
+int cuda_fail(cudaError_t e, const char *what) {
+    g_last_cuda_error = std::string(what) + ": " + cudaGetErrorString(e);
+    return MG_ECUDA;
+}
+#define CU(expr)                                            \
+    do {                                                    \
+        cudaError_t e__ = (expr);                           \
+        if (e__ != cudaSuccess) return cuda_fail(e__, #expr); \
+    } while (0)
+#define MG(expr)                  \
+    do {                          \
+        int rc__ = (expr);        \
+        if (rc__ != MG_OK) return rc__; \
+    } while (0)
+
+inline void count_launch(mg_handle *h) {
+    if (h->capturing) h->capture_count++;
+    else h->launches++;
+}
+#define LAUNCH(h, kern, grid, block, smem, ...)                     \
+    do {                                                            \
+        kern<<<(grid), (block), (smem), (h)->stream>>>(__VA_ARGS__); \
+        count_launch(h);                                            \
+    } while (0)
+
+int dalloc(mg_handle *h, void **p, size_t bytes) {
+    bytes = std::max<size_t>(bytes, 16);
+    void *q = nullptr;
+    if (h->opt.alloc) {
+        q = h->opt.alloc(bytes, h->opt.alloc_ctx);
+        if (!q) return MG_ENOMEM;
+    } else {
+        cudaError_t e = cudaMalloc(&q, bytes);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            return MG_ENOMEM;
+        }
+    }
+    h->owned.push_back(q);
+    h->dev_bytes += (int64_t)bytes;
+    *p = q;
+    return MG_OK;
+}
+template <typename T>
+int dalloc_t(mg_handle *h, T **p, size_t count) {
+    return dalloc(h, reinterpret_cast<void **>(p), count * sizeof(T));
+}
+
+inline int grid_for(int64_t n, int per_block, int cap = 148 * 16) {
+    int64_t g = (n + per_block - 1) / per_block;
+    return (int)std::max<int64_t>(1, std::min<int64_t>(g, cap));
+}
+
+// ------------------------------------------------------------------------------------------------ BSR launch
+int launch_bsr(mg_handle *h, const Level &L, BsrArgs a) {
+    a.row_ptr = L.row_ptr;
+    a.col_idx = L.col_idx;
+    a.vals = L.vals;
+    a.dinv = L.dinv;
+    a.n_brows = L.n_brows;
+    if (L.n_brows == 0) return MG_OK;
+    switch (h->b) {
+#define BSR_CASE(B)                                                                                          \
+    case B: {                                                                                                \
+        const int grid = (int)((L.n_brows + BsrCfg<B>::G - 1) / BsrCfg<B>::G);                                \
+        LAUNCH(h, bsr_fused_kernel<B>, grid, BsrCfg<B>::THREADS, 0, a);                                       \
+        break;                                                                                               \
+    }
+        BSR_CASE(6)
+        BSR_CASE(12)
+        BSR_CASE(36)
+#undef BSR_CASE
+        default: {
+            const int grid = (int)((L.n_brows + 3) / 4);
+            LAUNCH(h, bsr_fused_generic_kernel, grid, 128, 0, a, h->b);
+        }
+    }
+    CU(cudaGetLastError());
+    return MG_OK;
+}
+
+int spmv(mg_handle *h, const Level &L, const double *x, double *y, const int *done = nullptr) {
+    BsrArgs a{};
+    a.mode = MODE_SPMV;
+    a.vin = x;
+    a.out = y;
+    a.done = done;
+    return launch_bsr(h, L, a);
+}
+int residual(mg_handle *h, const Level &L, const double *rhs, const double *x, double *r, const int *done = nullptr) {
+    BsrArgs a{};
+    a.mode = MODE_RESID;
+    a.vin = x;
+    a.rin = rhs;
+    a.out = r;
+    a.done = done;
+    return launch_bsr(h, L, a);
+}
+// dout = c_z * Dinv rin ; if xacc: xacc += dout
+int pbj(mg_handle *h, const Level &L, const double *rin, double *dout, double c_z, double *xacc = nullptr,
+        const int *done = nullptr) {
+    BsrArgs a{};
+    a.mode = MODE_PBJ;
+    a.rin = rin;
+    a.dout = dout;
+    a.c_z = c_z;
+    a.x = xacc;
+    a.flags = xacc ? F_FINAL_X : 0;
+    a.done = done;
+    return launch_bsr(h, L, a);
+}
+int sweep(mg_handle *h, const Level &L, const double *vin, const double *rin, double *rout, double *x, double *dout,
+          double c_d, double c_z, int flags) {
+    BsrArgs a{};
+    a.mode = MODE_SWEEP;
+    a.vin = vin;
+    a.rin = rin;
+    a.out = rout;
+    a.x = x;
+    a.dout = dout;
+    a.c_d = c_d;
+    a.c_z = c_z;
+    a.flags = flags;
+    return launch_bsr(h, L, a);
+}
+
+// ------------------------------------------------------------------------------------------------ reductions
+// out[0] = <a, b> via the handle's scratch reduction (device result).
+int dot_dev(mg_handle *h, const double *a, const double *b, int64_t n, double *out) {
+    const int grid = grid_for(n / 2 + 1, 256 * 4, 1024);
+    LAUNCH(h, dot_multi_kernel, dim3(grid, 1), 256, 0, a, (int64_t)0, b, n, h->red_partial, h->red_counter, out,
+           (const int *)nullptr);
+    CU(cudaGetLastError());
+    return MG_OK;
+}
+int dot_host(mg_handle *h, const double *a, const double *b, int64_t n, double *result) {
+    MG(dot_dev(h, a, b, n, h->red_out));
+    CU(cudaMemcpyAsync(h->pinned_d, h->red_out, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    *result = h->pinned_d[0];
+    return MG_OK;
+}
+int scale_div(mg_handle *h, const double *src, double *dst, int64_t n, const double *denom, const int *done) {
+    LAUNCH(h, scale_div_kernel, grid_for(n, 256), 256, 0, src, dst, n, denom, done);
+    CU(cudaGetLastError());
+    return MG_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ smoothers
+struct Cheb {
+    double theta, delta, sigma1;
+};
+inline Cheb cheb_of(const Level &L) {
+    Cheb c;
+    c.theta = 0.5 * (L.lam_max + L.lam_min);
+    c.delta = 0.5 * (L.lam_max - L.lam_min);
+    c.sigma1 = c.theta / c.delta;
+    return c;
+}
+
+// nu >= 0 sweeps from a zero guess: x = x_nu, L.r = rhs - A x_nu (the residual carried by the recurrence).
+int presmooth(mg_handle *h, Level &L, const double *rhs, double *x, int nu) {
+    const size_t bytes = (size_t)L.nvec * sizeof(double);
+    if (nu <= 0) {
+        CU(cudaMemsetAsync(x, 0, bytes, h->stream));
+        CU(cudaMemcpyAsync(L.r, rhs, bytes, cudaMemcpyDeviceToDevice, h->stream));
+        return MG_OK;
+    }
+    const Cheb c = cheb_of(L);
+    MG(pbj(h, L, rhs, L.d[0], 1.0 / c.theta));  // d_0 = D^-1 r_0 / theta, r_0 = rhs
+    double rho = 1.0 / c.sigma1;
+    for (int k = 0; k < nu; ++k) {
+        const double rho_new = 1.0 / (2.0 * c.sigma1 - rho);
+        int flags = (k == 0) ? F_SET_X : F_UPD_X;
+        if (k < nu - 1) flags |= F_NEED_D;
+        MG(sweep(h, L, L.d[k & 1], k == 0 ? rhs : L.r, L.r, x, L.d[(k + 1) & 1], rho_new * rho, 2.0 * rho_new / c.delta,
+                 flags));
+        rho = rho_new;
+    }
+    return MG_OK;
+}
+
+// nu >= 1 sweeps from the guess x whose residual update is L.r - A v (v = correction just added to x, or x itself
+// with L.r = rhs).  v must not alias x.
+int postsmooth(mg_handle *h, Level &L, const double *v, double *x, int nu) {
+    if (nu <= 0) return MG_OK;
+    const Cheb c = cheb_of(L);
+    MG(sweep(h, L, v, L.r, L.r, x, L.d[0], 0.0, 1.0 / c.theta, F_NEED_D | (nu == 1 ? F_FINAL_X : 0)));
+    double rho = 1.0 / c.sigma1;
+    for (int k = 0; k + 1 < nu; ++k) {
+        const double rho_new = 1.0 / (2.0 * c.sigma1 - rho);
+        const int flags = F_UPD_X | F_NEED_D | (k == nu - 2 ? F_FINAL_X : 0);
+        MG(sweep(h, L, L.d[k & 1], L.r, L.r, x, L.d[(k + 1) & 1], rho_new * rho, 2.0 * rho_new / c.delta, flags));
+        rho = rho_new;
+    }
+    return MG_OK;
+}
+
+int restrict_to(mg_handle *h, int l, const double *rf, double *rc) {
+    const Level &L = h->lev[l];
+    const int64_t plane = (int64_t)h->n_pol * h->b;
+    LAUNCH(h, restrict_kernel, grid_for(plane * (L.n_phi / 2), 256), 256, 0, rf, rc, plane, L.n_phi, (const int *)nullptr);
+    CU(cudaGetLastError());
+    return MG_OK;
+}
+int prolong_add(mg_handle *h, int l, const double *ec, double *xf, double *pe) {
+    const Level &L = h->lev[l];
+    const int64_t plane = (int64_t)h->n_pol * h->b;
+    LAUNCH(h, prolong_add_kernel, grid_for(plane * L.n_phi, 256), 256, 0, ec, xf, pe, plane, L.n_phi, (const int *)nullptr);
+    CU(cudaGetLastError());
+    return MG_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ GMRES engine
+int gmres_alloc(mg_handle *h, Gmres &G, int64_t n, int m, int maxit, bool flexible) {
+    G.n = n;
+    G.m = m;
+    G.maxit = maxit;
+    G.flexible = flexible;
+    G.stride = (n + 31) / 32 * 32;
+    G.red_grid = grid_for(n / 2 + 1, 256 * 4, 256);
+    MG(dalloc_t(h, &G.V, (size_t)G.stride * (m + 1)));
+    if (flexible) MG(dalloc_t(h, &G.Z, (size_t)G.stride * m));
+    const int axpy_grid = (int)((n / 2 + 256) / 256);
+    MG(dalloc_t(h, &G.partial, (size_t)std::max((m + 1) * G.red_grid, axpy_grid)));
+    MG(dalloc_t(h, &G.counter, (size_t)(m + 2)));
+    CU(cudaMemsetAsync(G.counter, 0, sizeof(unsigned) * (m + 2), h->stream));
+    GmresDev &d = G.dev;
+    d.m = m;
+    d.maxit = maxit;
+    MG(dalloc_t(h, &d.H, (size_t)(m + 1) * m));
+    MG(dalloc_t(h, &d.cs, (size_t)m));
+    MG(dalloc_t(h, &d.sn, (size_t)m));
+    MG(dalloc_t(h, &d.g, (size_t)m + 1));
+    MG(dalloc_t(h, &d.y, (size_t)m));
+    MG(dalloc_t(h, &d.h1, (size_t)m + 1));
+    MG(dalloc_t(h, &d.h2, (size_t)m + 1));
+    MG(dalloc_t(h, &d.nrm2, 1));
+    MG(dalloc_t(h, &d.hnext, 1));
+    MG(dalloc_t(h, &d.tol, 1));
+    MG(dalloc_t(h, &d.hist, (size_t)maxit + 2));
+    MG(dalloc_t(h, &d.status, 4));
+    CU(cudaMemsetAsync(d.status, 0, 4 * sizeof(int), h->stream));
+    G.ready = true;
+    return MG_OK;
+}
+
+// tol = rtol * ||rhs||, iteration counters reset.
+int gmres_start(mg_handle *h, Gmres &G, const double *rhs, double rtol) {
+    LAUNCH(h, dot_multi_kernel, dim3(G.red_grid, 1), 256, 0, rhs, (int64_t)0, rhs, G.n, G.partial, G.counter,
+           G.dev.nrm2, (const int *)nullptr);
+    LAUNCH(h, gmres_set_tol_kernel, 1, 1, 0, G.dev, rtol);
+    CU(cudaGetLastError());
+    return MG_OK;
+}
+// V[0] holds the residual r: beta = ||r||, stop test, g = beta e_1, V[0] /= beta.
+int gmres_cycle_begin(mg_handle *h, Gmres &G) {
+    const int *done = G.dev.status;
+    LAUNCH(h, dot_multi_kernel, dim3(G.red_grid, 1), 256, 0, G.V, (int64_t)0, G.V, G.n, G.partial, G.counter, G.dev.nrm2,
+           done);
+    LAUNCH(h, gmres_begin_kernel, 1, 1, 0, G.dev);
+    MG(scale_div(h, G.V, G.V, G.n, G.dev.hnext, done));
+    return MG_OK;
+}
+// V[j+1] holds w = A M v_j: two classical Gram-Schmidt passes against V[0..j], Hessenberg column, v_{j+1}.
+int gmres_orth(mg_handle *h, Gmres &G, int j) {
+    const int *done = G.dev.status;
+    double *w = G.V + (size_t)(j + 1) * G.stride;
+    const int axpy_grid = (int)((G.n / 2 + 256) / 256);
+    for (int pass = 0; pass < 2; ++pass) {
+        double *hh = pass == 0 ? G.dev.h1 : G.dev.h2;
+        LAUNCH(h, dot_multi_kernel, dim3(G.red_grid, j + 1), 256, 0, G.V, G.stride, w, G.n, G.partial, G.counter, hh,
+               done);
+        LAUNCH(h, axpy_multi_kernel, axpy_grid, 256, 0, G.V, G.stride, j + 1, (const int *)nullptr, hh, -1.0, w, G.n,
+               G.partial, G.counter + G.m + 1, pass == 1 ? G.dev.nrm2 : (double *)nullptr, done);
+    }
+    LAUNCH(h, gmres_update_kernel, 1, 1, 0, G.dev, j);
+    MG(scale_div(h, w, w, G.n, G.dev.hnext, done));
+    CU(cudaGetLastError());
+    return MG_OK;
+}
+// y = H^-1 g ; out += sum_i y_i B_i  (B = Z for flexible, V otherwise)
+int gmres_cycle_end(mg_handle *h, Gmres &G, double *out) {
+    LAUNCH(h, gmres_solve_y_kernel, 1, 1, 0, G.dev);
+    const int axpy_grid = (int)((G.n / 2 + 256) / 256);
+    LAUNCH(h, axpy_multi_kernel, axpy_grid, 256, 0, G.flexible ? G.Z : G.V, G.stride, G.m, G.dev.status + 1, G.dev.y, 1.0,
+           out, G.n, G.partial, G.counter + G.m + 1, (double *)nullptr, (const int *)nullptr);
+    CU(cudaGetLastError());
+    return MG_OK;
+}
+int read_status(mg_handle *h, Gmres &G, int st[4]) {
+    CU(cudaMemcpyAsync(h->pinned, G.dev.status, 4 * sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    for (int i = 0; i < 4; ++i) st[i] = h->pinned[i];
+    return MG_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ coarse solve
+int coarse_cycle_enqueue(mg_handle *h) {
+    Level &L = h->lev.back();
+    Gmres &G = h->coarse;
+    const int *done = G.dev.status;
+    MG(residual(h, L, L.rhs, L.x, G.V, done));
+    MG(gmres_cycle_begin(h, G));
+    for (int j = 0; j < G.m; ++j) {
+        MG(pbj(h, L, G.V + (size_t)j * G.stride, L.d[0], 1.0, nullptr, done));
+        MG(spmv(h, L, L.d[0], G.V + (size_t)(j + 1) * G.stride, done));
+        MG(gmres_orth(h, G, j));
+    }
+    CU(cudaMemsetAsync(L.d[1], 0, (size_t)L.nvec * sizeof(double), h->stream));
+    MG(gmres_cycle_end(h, G, L.d[1]));
+    MG(pbj(h, L, L.d[1], L.d[0], 1.0, L.x));  // e += D^-1 (V y)
+    return MG_OK;
+}
+
+// Solve A_{L-1} x = rhs on the coarsest level's own buffers (L.rhs -> L.x), zero guess.
+int coarse_solve_internal(mg_handle *h) {
+    Level &L = h->lev.back();
+    if (h->opt.coarse_mode == 1) {
+        h->coarse_iters_last = h->opt.coarse_fixed_sweeps;
+        h->coarse_iters_total += h->coarse_iters_last;
+        return presmooth(h, L, L.rhs, L.x, h->opt.coarse_fixed_sweeps);
+    }
+    Gmres &G = h->coarse;
+    if (!G.ready || G.m != h->opt.coarse_restart || G.maxit != h->opt.coarse_maxit) {
+        if (h->coarse_graph) {
+            cudaGraphExecDestroy(h->coarse_graph);
+            h->coarse_graph = nullptr;
+        }
+        MG(gmres_alloc(h, G, L.nvec, h->opt.coarse_restart, h->opt.coarse_maxit, false));
+    }
+    CU(cudaMemsetAsync(L.x, 0, (size_t)L.nvec * sizeof(double), h->stream));
+    MG(gmres_start(h, G, L.rhs, h->opt.coarse_rtol));
+    if (h->opt.use_graphs && !h->coarse_graph) {
+        cudaGraph_t graph = nullptr;
+        if (!h->cap_stream) CU(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
+        cudaStream_t user_stream = h->stream;
+        CU(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
+        h->stream = h->cap_stream;
+        h->capturing = true;
+        h->capture_count = 0;
+        const int rc = coarse_cycle_enqueue(h);
+        h->capturing = false;
+        h->stream = user_stream;
+        cudaError_t e = cudaStreamEndCapture(h->cap_stream, &graph);
+        if (rc != MG_OK) {
+            if (graph) cudaGraphDestroy(graph);
+            return rc;
+        }
+        if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture");
+        h->coarse_graph_kernels = h->capture_count;
+        e = cudaGraphInstantiate(&h->coarse_graph, graph, 0);
+        cudaGraphDestroy(graph);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaGraphInstantiate");
+    }
+    int st[4] = {0, 0, 0, 0};
+    do {
+        if (h->coarse_graph) {
+            CU(cudaGraphLaunch(h->coarse_graph, h->stream));
+            h->launches += h->coarse_graph_kernels;
+        } else {
+            MG(coarse_cycle_enqueue(h));
+        }
+        MG(read_status(h, G, st));
+    } while (!st[0]);
+    h->coarse_iters_last = st[2];
+    h->coarse_iters_total += st[2];
+    return MG_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ V-cycle
+int vcycle_internal(mg_handle *h, const double *r, double *z) {
+    const int Lc = h->n_levels - 1;
+    if (Lc == 0) {
+        Level &L = h->lev[0];
+        CU(cudaMemcpyAsync(L.rhs, r, (size_t)L.nvec * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
+        MG(coarse_solve_internal(h));
+        CU(cudaMemcpyAsync(z, L.x, (size_t)L.nvec * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
+        return MG_OK;
+    }
+    for (int l = 0; l < Lc; ++l) {
+        Level &L = h->lev[l];
+        const double *rhs = (l == 0) ? r : L.rhs;
+        double *x = (l == 0) ? z : L.x;
+        MG(presmooth(h, L, rhs, x, h->opt.nu_pre));
+        MG(restrict_to(h, l, L.r, h->lev[l + 1].rhs));
+    }
+    MG(coarse_solve_internal(h));
+    for (int l = Lc - 1; l >= 0; --l) {
+        Level &L = h->lev[l];
+        double *x = (l == 0) ? z : L.x;
+        MG(prolong_add(h, l, h->lev[l + 1].x, x, h->opt.nu_post > 0 ? L.pe : nullptr));
+        MG(postsmooth(h, L, L.pe, x, h->opt.nu_post));
+    }
+    return MG_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ setup pieces
+int power_rho(mg_handle *h, Level &L, int iters, double *rho_out) {
+    LAUNCH(h, hashed_start_kernel, grid_for(L.nvec, 256), 256, 0, L.x, L.nvec);
+    double nrm2 = 0.0;
+    MG(dot_host(h, L.x, L.x, L.nvec, &nrm2));
+    if (!(nrm2 > 0.0)) {
+        *rho_out = 1.0;
+        return MG_OK;
+    }
+    LAUNCH(h, axpby_kernel, grid_for(L.nvec, 256), 256, 0, 1.0 / std::sqrt(nrm2), L.x, 0.0, L.x, L.nvec);
+    double rho = 0.0;
+    for (int it = 0; it < iters; ++it) {
+        MG(spmv(h, L, L.x, L.r));
+        MG(pbj(h, L, L.r, L.d[0], 1.0));
+        MG(dot_host(h, L.d[0], L.d[0], L.nvec, &nrm2));
+        rho = std::sqrt(nrm2);
+        if (!(rho > 0.0)) break;
+        LAUNCH(h, axpby_kernel, grid_for(L.nvec, 256), 256, 0, 1.0 / rho, L.d[0], 0.0, L.x, L.nvec);
+    }
+    CU(cudaGetLastError());
+    *rho_out = rho;
+    return MG_OK;
+}
+
+void set_bounds(mg_handle *h, Level &L) {
+    L.lam_min = h->opt.cheb_lo * L.rho_est;
+    L.lam_max = h->opt.cheb_hi * L.rho_est;
+}
+
+// Host symbolic phase of the Galerkin product: the coarse pattern in closed form from the fine pattern.
+void galerkin_symbolic(const Level &F, int n_pol, std::vector<int64_t> &crow_ptr, std::vector<int32_t> &ccol,
+                       std::vector<int64_t> &crow_of_block) {
+    const int n_f = F.n_phi, n_c = n_f / 2;
+    crow_ptr.assign((size_t)n_c * n_pol + 1, 0);
+    ccol.clear();
+    crow_of_block.clear();
+    std::vector<int64_t> cand;
+    for (int K = 0; K < n_c; ++K) {
+        int ks[3] = {(2 * K - 1 + n_f) % n_f, 2 * K, (2 * K + 1) % n_f};
+        int nk = 0, kk[3];
+        for (int a = 0; a < 3; ++a) {
+            bool dup = false;
+            for (int a2 = 0; a2 < nk; ++a2) dup |= (kk[a2] == ks[a]);
+            if (!dup) kk[nk++] = ks[a];
+        }
+        for (int i = 0; i < n_pol; ++i) {
+            cand.clear();
+            for (int a = 0; a < nk; ++a) {
+                const int64_t If = (int64_t)kk[a] * n_pol + i;
+                for (int64_t p = F.h_row_ptr[If]; p < F.h_row_ptr[If + 1]; ++p) {
+                    const int64_t J = F.h_col_idx[p];
+                    const int m = (int)(J / n_pol);
+                    const int64_t j = J % n_pol;
+                    if ((m & 1) == 0) {
+                        cand.push_back((int64_t)(m / 2) * n_pol + j);
+                    } else {
+                        cand.push_back((int64_t)((m - 1) / 2) * n_pol + j);
+                        cand.push_back((int64_t)(((m + 1) / 2) % n_c) * n_pol + j);
+                    }
+                }
+            }
+            std::sort(cand.begin(), cand.end());
+            cand.erase(std::unique(cand.begin(), cand.end()), cand.end());
+            const int64_t Ic = (int64_t)K * n_pol + i;
+            for (int64_t c : cand) {
+                ccol.push_back((int32_t)c);
+                crow_of_block.push_back(Ic);
+            }
+            crow_ptr[Ic + 1] = (int64_t)ccol.size();
+        }
+    }
+}
+
+int alloc_level_vectors(mg_handle *h, Level &L) {
+    const size_t n = (size_t)L.nvec + 2;
+    MG(dalloc_t(h, &L.x, n));
+    MG(dalloc_t(h, &L.r, n));
+    MG(dalloc_t(h, &L.d[0], n));
+    MG(dalloc_t(h, &L.d[1], n));
+    MG(dalloc_t(h, &L.pe, n));
+    MG(dalloc_t(h, &L.rhs, n));
+    return MG_OK;
+}
+
+int setup_level_pbj(mg_handle *h, Level &L) {
+    const int b = h->b;
+    MG(dalloc_t(h, &L.diag_pos, (size_t)L.n_brows));
+    unsigned long long *err = nullptr;
+    MG(dalloc_t(h, &err, 3));
+    CU(cudaMemsetAsync(err, 0xff, 3 * sizeof(unsigned long long), h->stream));
+    LAUNCH(h, check_pattern_kernel, grid_for(L.n_brows, 256, 1 << 30), 256, 0, L.row_ptr, L.col_idx, L.n_brows, L.diag_pos,
+           err, err + 1);
+    unsigned long long herr[3];
+    CU(cudaMemcpyAsync(herr, err, sizeof(herr), cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    if (herr[0] != ~0ull) return MG_EINVAL;
+    if (herr[1] != ~0ull) return MG_ESINGULAR;
+    MG(dalloc_t(h, &L.dinv, (size_t)L.n_brows * b * b));
+    const size_t smem = sizeof(double) * (size_t)(2 * b * b + b);
+    if (smem > 48 * 1024)
+        CU(cudaFuncSetAttribute(invert_blocks_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (L.n_brows > 0) LAUNCH(h, invert_blocks_kernel, (unsigned)L.n_brows, 128, smem, L.vals, L.diag_pos, b, L.dinv, err + 2);
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(herr, err, sizeof(herr), cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    if (herr[2] != ~0ull) return MG_ESINGULAR;
+    return MG_OK;
+}
+
+int build_coarse_level(mg_handle *h, int l) {
+    Level &F = h->lev[l];
+    Level &C = h->lev[l + 1];
+    const int b = h->b;
+    if (F.h_row_ptr.empty()) {
+        F.h_row_ptr.resize((size_t)F.n_brows + 1);
+        F.h_col_idx.resize((size_t)F.nnzb);
+        CU(cudaMemcpyAsync(F.h_row_ptr.data(), F.row_ptr, sizeof(int64_t) * (F.n_brows + 1), cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaMemcpyAsync(F.h_col_idx.data(), F.col_idx, sizeof(int32_t) * F.nnzb, cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+    }
+    std::vector<int64_t> crow_of_block;
+    galerkin_symbolic(F, h->n_pol, C.h_row_ptr, C.h_col_idx, crow_of_block);
+    C.n_phi = F.n_phi / 2;
+    C.n_brows = (int64_t)C.n_phi * h->n_pol;
+    C.nvec = C.n_brows * b;
+    C.nnzb = (int64_t)C.h_col_idx.size();
+    int64_t *d_rp = nullptr, *d_rob = nullptr;
+    int32_t *d_ci = nullptr;
+    double *d_v = nullptr;
+    MG(dalloc_t(h, &d_rp, (size_t)C.n_brows + 1));
+    MG(dalloc_t(h, &d_ci, (size_t)C.nnzb));
+    MG(dalloc_t(h, &d_v, (size_t)C.nnzb * b * b));
+    cudaError_t e = cudaMalloc(&d_rob, sizeof(int64_t) * std::max<int64_t>(C.nnzb, 1));
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return MG_ENOMEM;
+    }
+    CU(cudaMemcpyAsync(d_rp, C.h_row_ptr.data(), sizeof(int64_t) * (C.n_brows + 1), cudaMemcpyHostToDevice, h->stream));
+    CU(cudaMemcpyAsync(d_ci, C.h_col_idx.data(), sizeof(int32_t) * C.nnzb, cudaMemcpyHostToDevice, h->stream));
+    CU(cudaMemcpyAsync(d_rob, crow_of_block.data(), sizeof(int64_t) * C.nnzb, cudaMemcpyHostToDevice, h->stream));
+    if (C.nnzb > 0)
+        LAUNCH(h, galerkin_numeric_kernel, (unsigned)C.nnzb, 128, 0, F.row_ptr, F.col_idx, F.vals, d_rob, d_ci, d_v, h->n_pol,
+               F.n_phi, b);
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(h->stream));
+    cudaFree(d_rob);
+    C.row_ptr = d_rp;
+    C.col_idx = d_ci;
+    C.vals = d_v;
+    return MG_OK;
+}
+
+bool level_ok(mg_handle *h, int level) { return h && level >= 0 && level < h->n_levels; }
+
+}  // namespace
+
+// ================================================================================================ C ABI
+extern "C" {
+
+int mg_options_default(mg_options *o) {
+    if (!o) return MG_EINVAL;
+    std::memset(o, 0, sizeof(*o));
+    o->nu_pre = 2;
+    o->nu_post = 2;
+    o->cheb_lo = 0.1;
+    o->cheb_hi = 1.1;
+    o->eig_iters = 20;
+    o->coarse_mode = 0;
+    o->coarse_rtol = 1e-10;
+    o->coarse_restart = 50;
+    o->coarse_maxit = 20000;
+    o->coarse_fixed_sweeps = 8;
+    o->restart = 100;
+    o->maxit = 400;
+    o->block_layout = 0;
+    o->use_graphs = 1;
+    return MG_OK;
+}
+
+static int validate_options(const mg_options &o) {
+    if (o.nu_pre < 0 || o.nu_post < 0 || o.eig_iters < 1) return MG_EINVAL;
+    if (!(o.cheb_lo > 0.0) || !(o.cheb_hi > o.cheb_lo)) return MG_EINVAL;
+    if (o.coarse_mode < 0 || o.coarse_mode > 1 || !(o.coarse_rtol > 0.0)) return MG_EINVAL;
+    if (o.coarse_restart < 1 || o.coarse_maxit < 1 || o.coarse_fixed_sweeps < 0) return MG_EINVAL;
+    if (o.restart < 1 || o.maxit < 1 || o.block_layout != 0) return MG_EINVAL;
+    return MG_OK;
+}
+
+int mg_destroy(mg_handle *h) {
+    if (!h) return MG_EINVAL;
+    cudaStreamSynchronize(h->stream);
+    if (h->coarse_graph) cudaGraphExecDestroy(h->coarse_graph);
+    if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+    for (void *p : h->owned) {
+        if (h->opt.free) h->opt.free(p, h->opt.alloc_ctx);
+        else if (!h->opt.alloc) cudaFree(p);
+    }
+    if (h->pinned) cudaFreeHost(h->pinned);
+    if (h->pinned_d) cudaFreeHost(h->pinned_d);
+    delete h;
+    return MG_OK;
+}
+
+int mg_setup(mg_handle **out, const int64_t *row_ptr, const int32_t *col_idx, const double *vals, int b, int n_pol,
+             int n_phi, int levels, const mg_options *opt, void *cuda_stream) {
+    if (!out) return MG_EINVAL;
+    *out = nullptr;
+    if (!row_ptr || !col_idx || !vals) return MG_EINVAL;
+    if (b < 1 || b > 64 || n_pol < 1 || n_phi < 1 || levels < 1 || levels > 30) return MG_EINVAL;
+    if (n_phi % (1 << (levels - 1)) != 0) return MG_EINVAL;
+    mg_options o;
+    if (opt) o = *opt; else mg_options_default(&o);
+    if (validate_options(o) != MG_OK) return MG_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        g_last_cuda_error = "no CUDA device: libmgtoroidal has no CPU fallback";
+        return MG_ECUDA;
+    }
+    mg_handle *h = new mg_handle();
+    h->opt = o;
+    h->b = b;
+    h->n_pol = n_pol;
+    h->n_phi = n_phi;
+    h->n_levels = levels;
+    h->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    h->lev.resize(levels);
+    int rc = MG_OK;
+    auto fail = [&](int code) {
+        mg_destroy(h);
+        return code;
+    };
+    if (cudaMallocHost(&h->pinned, 8 * sizeof(int)) != cudaSuccess || cudaMallocHost(&h->pinned_d, 8 * sizeof(double)) != cudaSuccess)
+        return fail(cuda_fail(cudaGetLastError(), "cudaMallocHost"));
+    if ((rc = dalloc_t(h, &h->red_partial, 2048)) != MG_OK) return fail(rc);
+    if ((rc = dalloc_t(h, &h->red_out, 8)) != MG_OK) return fail(rc);
+    if ((rc = dalloc_t(h, &h->red_counter, 8)) != MG_OK) return fail(rc);
+    if (cudaMemsetAsync(h->red_counter, 0, 8 * sizeof(unsigned), h->stream) != cudaSuccess)
+        return fail(cuda_fail(cudaGetLastError(), "cudaMemsetAsync"));
+
+    Level &L0 = h->lev[0];
+    L0.n_phi = n_phi;
+    L0.n_brows = (int64_t)n_pol * n_phi;
+    L0.nvec = L0.n_brows * b;
+    L0.row_ptr = row_ptr;
+    L0.col_idx = col_idx;
+    L0.vals = vals;
+    int64_t ends[2] = {0, 0};
+    if (cudaMemcpyAsync(&ends[0], row_ptr, sizeof(int64_t), cudaMemcpyDeviceToHost, h->stream) != cudaSuccess ||
+        cudaMemcpyAsync(&ends[1], row_ptr + L0.n_brows, sizeof(int64_t), cudaMemcpyDeviceToHost, h->stream) != cudaSuccess ||
+        cudaStreamSynchronize(h->stream) != cudaSuccess)
+        return fail(cuda_fail(cudaGetLastError(), "read row_ptr"));
+    if (ends[0] != 0 || ends[1] < L0.n_brows) return fail(MG_EINVAL);
+    L0.nnzb = ends[1];
+
+    for (int l = 0; l < levels; ++l) {
+        Level &L = h->lev[l];
+        if ((rc = setup_level_pbj(h, L)) != MG_OK) return fail(rc);
+        if ((rc = alloc_level_vectors(h, L)) != MG_OK) return fail(rc);
+        if ((rc = power_rho(h, L, o.eig_iters, &L.rho_est)) != MG_OK) return fail(rc);
+        set_bounds(h, L);
+        if (l + 1 < levels && (rc = build_coarse_level(h, l)) != MG_OK) return fail(rc);
+    }
+    if (cudaStreamSynchronize(h->stream) != cudaSuccess) return fail(cuda_fail(cudaGetLastError(), "setup sync"));
+    *out = h;
+    return MG_OK;
+}
+
+int mg_update_options(mg_handle *h, const mg_options *opt) {
+    if (!h || !opt) return MG_EINVAL;
+    mg_options o = *opt;
+    o.alloc = h->opt.alloc;
+    o.free = h->opt.free;
+    o.alloc_ctx = h->opt.alloc_ctx;
+    o.eig_iters = h->opt.eig_iters;
+    o.block_layout = h->opt.block_layout;
+    if (validate_options(o) != MG_OK) return MG_EINVAL;
+    const bool bounds = (o.cheb_lo != h->opt.cheb_lo) || (o.cheb_hi != h->opt.cheb_hi);
+    h->opt = o;
+    if (bounds)
+        for (auto &L : h->lev) set_bounds(h, L);
+    return MG_OK;
+}
+
+int mg_vcycle(mg_handle *h, const double *r, double *z) {
+    if (!h || !r || !z || r == z) return MG_EINVAL;
+    return vcycle_internal(h, r, z);
+}
+
+int mg_solve(mg_handle *h, const double *rhs, double *x, double rtol, int x_is_initial_guess, mg_solve_info *info) {
+    if (!h || !rhs || !x || rhs == x || !(rtol > 0.0)) return MG_EINVAL;
+    Level &L = h->lev[0];
+    Gmres &G = h->outer;
+    const int64_t n = L.nvec;
+    const size_t bytes = (size_t)n * sizeof(double);
+    if (!G.ready || G.m != h->opt.restart || G.maxit != h->opt.maxit)
+        MG(gmres_alloc(h, G, n, h->opt.restart, h->opt.maxit, true));
+    h->coarse_iters_total = 0;
+    if (!x_is_initial_guess) CU(cudaMemsetAsync(x, 0, bytes, h->stream));
+    MG(gmres_start(h, G, rhs, rtol));
+    CU(cudaMemcpyAsync(h->pinned_d, G.dev.nrm2, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    const double bnorm = std::sqrt(std::max(h->pinned_d[0], 0.0));
+    int st[4] = {0, 0, 0, 0};
+    if (bnorm == 0.0) {
+        CU(cudaMemsetAsync(x, 0, bytes, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+        if (info) {
+            info->iters = 0;
+            info->converged = 1;
+            info->rel_res = 0.0;
+            info->coarse_iters_total = 0;
+            if (info->hist && info->hist_len > 0) info->hist[0] = 0.0;
+            info->hist_len = (info->hist && info->hist_len > 0) ? 1 : 0;
+        }
+        return MG_OK;
+    }
+    while (true) {
+        MG(residual(h, L, rhs, x, G.V));
+        MG(gmres_cycle_begin(h, G));
+        MG(read_status(h, G, st));
+        if (st[0]) break;
+        for (int j = 0; j < G.m; ++j) {
+            double *zj = G.Z + (size_t)j * G.stride;
+            MG(vcycle_internal(h, G.V + (size_t)j * G.stride, zj));
+            MG(spmv(h, L, zj, G.V + (size_t)(j + 1) * G.stride));
+            MG(gmres_orth(h, G, j));
+            MG(read_status(h, G, st));
+            if (st[0]) break;
+        }
+        MG(gmres_cycle_end(h, G, x));
+        if (st[0]) break;
+    }
+    // true residual
+    MG(residual(h, L, rhs, x, L.r));
+    double rn2 = 0.0;
+    MG(dot_host(h, L.r, L.r, n, &rn2));
+    if (info) {
+        info->iters = st[2];
+        info->converged = st[3];
+        info->rel_res = std::sqrt(std::max(rn2, 0.0)) / bnorm;
+        info->coarse_iters_total = h->coarse_iters_total;
+        int cnt = 0;
+        if (info->hist && info->hist_len > 0) {
+            cnt = std::min(info->hist_len, st[2] + 1);
+            CU(cudaMemcpy(info->hist, G.dev.hist, sizeof(double) * cnt, cudaMemcpyDeviceToHost));
+            for (int i = 0; i < cnt; ++i) info->hist[i] /= bnorm;
+        }
+        info->hist_len = cnt;
+    }
+    return MG_OK;
+}
+
+int mg_solve_host(mg_handle *h, const double *rhs_host, double *x_host, double rtol, int x_is_initial_guess,
+                  mg_solve_info *info) {
+    if (!h || !rhs_host || !x_host) return MG_EINVAL;
+    Level &L = h->lev[0];
+    const size_t bytes = (size_t)L.nvec * sizeof(double);
+    if (!h->d_rhs_host) {
+        MG(dalloc_t(h, &h->d_rhs_host, (size_t)L.nvec + 2));
+        MG(dalloc_t(h, &h->d_x_host, (size_t)L.nvec + 2));
+    }
+    CU(cudaMemcpyAsync(h->d_rhs_host, rhs_host, bytes, cudaMemcpyHostToDevice, h->stream));
+    if (x_is_initial_guess) CU(cudaMemcpyAsync(h->d_x_host, x_host, bytes, cudaMemcpyHostToDevice, h->stream));
+    MG(mg_solve(h, h->d_rhs_host, h->d_x_host, rtol, x_is_initial_guess, info));
+    CU(cudaMemcpyAsync(x_host, h->d_x_host, bytes, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    return MG_OK;
+}
+
+int mg_spmv(mg_handle *h, int level, const double *x, double *y) {
+    if (!level_ok(h, level) || !x || !y || x == y) return MG_EINVAL;
+    return spmv(h, h->lev[level], x, y);
+}
+
+int mg_residual(mg_handle *h, int level, const double *rhs, const double *x, double *r) {
+    if (!level_ok(h, level) || !rhs || !x || !r || x == r) return MG_EINVAL;
+    return residual(h, h->lev[level], rhs, x, r);
+}
+
+int mg_pbj_apply(mg_handle *h, int level, const double *r, double *z) {
+    if (!level_ok(h, level) || !r || !z) return MG_EINVAL;
+    return pbj(h, h->lev[level], r, z, 1.0);
+}
+
+int mg_smooth(mg_handle *h, int level, const double *rhs, double *x, int nu, int zero_guess) {
+    if (!level_ok(h, level) || !rhs || !x || nu < 0 || rhs == x) return MG_EINVAL;
+    Level &L = h->lev[level];
+    if (zero_guess) return presmooth(h, L, rhs, x, nu);
+    if (nu == 0) return MG_OK;
+    const size_t bytes = (size_t)L.nvec * sizeof(double);
+    CU(cudaMemcpyAsync(L.pe, x, bytes, cudaMemcpyDeviceToDevice, h->stream));   // v = x_0 (gathered copy)
+    CU(cudaMemcpyAsync(L.r, rhs, bytes, cudaMemcpyDeviceToDevice, h->stream));  // r = rhs, then r -= A x_0
+    return postsmooth(h, L, L.pe, x, nu);
+}
+
+int mg_restrict(mg_handle *h, int level, const double *r_fine, double *r_coarse) {
+    if (!level_ok(h, level) || level + 1 >= h->n_levels || !r_fine || !r_coarse) return MG_EINVAL;
+    return restrict_to(h, level, r_fine, r_coarse);
+}
+
+int mg_prolong_add(mg_handle *h, int level, const double *e_coarse, double *x_fine) {
+    if (!level_ok(h, level) || level + 1 >= h->n_levels || !e_coarse || !x_fine) return MG_EINVAL;
+    return prolong_add(h, level, e_coarse, x_fine, nullptr);
+}
+
+int mg_coarse_solve(mg_handle *h, const double *r, double *e, int *iters) {
+    if (!h || !r || !e) return MG_EINVAL;
+    Level &L = h->lev.back();
+    const size_t bytes = (size_t)L.nvec * sizeof(double);
+    CU(cudaMemcpyAsync(L.rhs, r, bytes, cudaMemcpyDeviceToDevice, h->stream));
+    MG(coarse_solve_internal(h));
+    CU(cudaMemcpyAsync(e, L.x, bytes, cudaMemcpyDeviceToDevice, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    if (iters) *iters = h->coarse_iters_last;
+    return MG_OK;
+}
+
+int mg_get_level(mg_handle *h, int level, int64_t *n_brows, int64_t *nnzb, const int64_t **row_ptr,
+                 const int32_t **col_idx, const double **vals, const double **dinv, double *rho_est, double *lam_min,
+                 double *lam_max) {
+    if (!level_ok(h, level)) return MG_EINVAL;
+    const Level &L = h->lev[level];
+    if (n_brows) *n_brows = L.n_brows;
+    if (nnzb) *nnzb = L.nnzb;
+    if (row_ptr) *row_ptr = L.row_ptr;
+    if (col_idx) *col_idx = L.col_idx;
+    if (vals) *vals = L.vals;
+    if (dinv) *dinv = L.dinv;
+    if (rho_est) *rho_est = L.rho_est;
+    if (lam_min) *lam_min = L.lam_min;
+    if (lam_max) *lam_max = L.lam_max;
+    return MG_OK;
+}
+
+int mg_copy_level_to_host(mg_handle *h, int level, int64_t *row_ptr_host, int32_t *col_idx_host, double *vals_host,
+                          double *dinv_host) {
+    if (!level_ok(h, level)) return MG_EINVAL;
+    const Level &L = h->lev[level];
+    const size_t bb = (size_t)h->b * h->b;
+    if (row_ptr_host)
+        CU(cudaMemcpyAsync(row_ptr_host, L.row_ptr, sizeof(int64_t) * (L.n_brows + 1), cudaMemcpyDeviceToHost, h->stream));
+    if (col_idx_host && L.nnzb > 0)
+        CU(cudaMemcpyAsync(col_idx_host, L.col_idx, sizeof(int32_t) * L.nnzb, cudaMemcpyDeviceToHost, h->stream));
+    if (vals_host && L.nnzb > 0)
+        CU(cudaMemcpyAsync(vals_host, L.vals, sizeof(double) * L.nnzb * bb, cudaMemcpyDeviceToHost, h->stream));
+    if (dinv_host && L.n_brows > 0)
+        CU(cudaMemcpyAsync(dinv_host, L.dinv, sizeof(double) * L.n_brows * bb, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    return MG_OK;
+}
+
+int mg_set_cheb_bounds(mg_handle *h, int level, double lam_min, double lam_max) {
+    if (!level_ok(h, level) || !(lam_min > 0.0) || !(lam_max > lam_min)) return MG_EINVAL;
+    h->lev[level].lam_min = lam_min;
+    h->lev[level].lam_max = lam_max;
+    return MG_OK;
+}
+
+int64_t mg_launch_count(mg_handle *h) { return h ? h->launches : -1; }
+int64_t mg_device_bytes(mg_handle *h) { return h ? h->dev_bytes : -1; }
+
+const char *mg_strerror(int code) {
+    switch (code) {
+        case MG_OK: return "ok";
+        case MG_EINVAL: return "invalid argument (shape, ordering, divisibility, NULL or aliased pointer, unsupported b)";
+        case MG_ENOMEM: return "out of memory";
+        case MG_ESINGULAR: return "a diagonal block is missing or singular";
+        case MG_ECUDA: return g_last_cuda_error.empty() ? "CUDA error" : g_last_cuda_error.c_str();
+        default: return "unknown error code";
+    }
+}
+
+const char *mg_version(void) { return "mg_toroidal 0.1.0 (sm_100a)"; }
+
+}  // extern "C"
