@@ -24,7 +24,11 @@ def small(name="C0", **kw):
     return make_workload(name, **kw)
 
 
+GPU_ONLY_OPTIONS = ("use_graphs",)   # launch mechanics of the CUDA library; no arithmetic meaning
+
+
 def oracle_hierarchy(w, **opt):
+    opt = {k: v for k, v in opt.items() if k not in GPU_ONLY_OPTIONS}
     return mg.setup(w.row_ptr, w.col_idx, w.vals, w.b, w.n_pol, w.n_phi, w.levels, mg.Options(**opt))
 
 
