@@ -1,0 +1,378 @@
+#!/usr/bin/env python
+"""bench.py -- FP64 MG-FGMRES solve time to rtol 1e-8 on one B200 (BASELINE.json metric), with the HBM
+roofline of the dominant kernel and the CPU oracle timed beside it.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C1] [--impl reference]
+
+A STEP is one complete ``mg_solve`` (FGMRES preconditioned by the toroidal semi-coarsening V-cycle, to
+rtol 1e-8) of one seeded synthetic right-hand side on the workload BASELINE.json's metric is quoted on
+(configs[1] "Medium": 2,000 poloidal nodes x 16 planes, b = 36, 4 levels).  The hierarchy (mg_setup) is built
+once, outside the timed region (it is the paper's lagged "refresh"), and reported in ``config``.
+
+* ``value``  = seconds per solve, device time between CUDA events inside the library with the right-hand
+  side already resident in HBM (``mg_solve_info.solve_ms``), MAX over ranks.
+* ``e2e``    = the same K solves timed around the public host-buffer call ``mg_solve_host`` (pinned host
+  rhs -> device, solve, x -> pinned host), CUDA events on the library's stream, MAX over ranks.
+* ``roofline`` = the kernel class with the largest share of the step: algorithmic bytes per launch
+  (paper_2506_16676_b200/traffic.py) / its mean CUDA-event duration, measured
+  in a short event-bracketed pass right after the timed steps, against MEASURED_PEAKS.json's HBM copy rate.
+* ``cpu_baseline`` = the oracle (oracle/, as it stands) timed on the host cores on a bounded sample and
+  extrapolated by algorithmic bytes to one solve.  A reported baseline, not the target.
+* N > 1: REPLICAS ONLY -- the path does not shard (north_star: one GPU); N independent solves.
+
+``--impl reference`` times the oracle alone (no GPU work) and prints the same line with "impl": "reference".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "mg_fgmres_solve_time_to_rtol_1e-8"
+UNIT = "s"
+RTOL = 1e-8
+# Extrapolation constants of the oracle arm when no GPU run is at hand (--impl reference runs first, on a fresh
+# box): FGMRES / coarse-GMRES iteration counts of one C1 solve, as measured by this library on a B200 in round 1
+# (the oracle was never run to convergence at this size: hours of CPU time).  Used ONLY to scale a measured
+# oracle GB/s to a solve; never an input or an expected value of any parity test.
+REFERENCE_COUNTS = {"C1": dict(outer_iters=186, coarse_iters=903027), "C0": dict(outer_iters=40, coarse_iters=40000)}
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+# ------------------------------------------------------------------------------------------------- helpers
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, device copy)"
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.path = index, None, None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "200", "-i", str(self.index)], stdout=open(self.path, "w"),
+                                         stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self) -> dict:
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        try:
+            for line in open(self.path):
+                f = [t.strip() for t in line.split(",")]
+                if len(f) < 7:
+                    continue
+                try:
+                    sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+                except ValueError:
+                    continue
+                for nm, v in zip(names, f[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+            os.unlink(self.path)
+        except Exception:
+            pass
+        if sm:
+            sm.sort()
+            out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=max(mx), power_w_max=max(pw), reasons=sorted(reasons),
+                       samples=len(sm))
+        return out
+
+
+def level_sizes(solver):
+    from paper_2506_16676_b200.traffic import LevelSize
+    out = []
+    for l in range(solver.levels):
+        g = solver.get_level(l)
+        out.append(LevelSize(n_brows=g["n_brows"], nnzb=g["nnzb"], b=solver.b))
+    return out
+
+
+def class_bytes(sizes, level, kind, restart_by_level):
+    """Algorithmic bytes of ONE launch of a (level, kind) class (traffic.py)."""
+    L = sizes[level]
+    if kind in ("spmv", "resid", "sweep", "sweep_nod", "pbj", "restrict", "prolong"):
+        return L.by_kind(kind)
+    if kind == "cycle":     # one whole restart cycle of the coarsest-level GMRES: m iterations, j = 0..m-1
+        m = restart_by_level.get(level, 1)
+        return sum(L.gmres_iteration(j) for j in range(m))
+    return 0                # orth / other: sized from the iteration counts (orth_bytes)
+
+
+# ------------------------------------------------------------------------------------------------- oracle arm
+def oracle_sample(w, seconds: float = 15.0):
+    """Time the oracle (as it stands) on a bounded sample of the workload: fine-level block SpMV and PBJ apply,
+    repeated for about ``seconds``.  Returns (GB/s of algorithmic bytes, seconds used, threads, description)."""
+    import numpy as np
+    from oracle import mg as oracle_mg
+    from paper_2506_16676_b200.traffic import LevelSize
+    L = oracle_mg.Level(n_phi=w.n_phi, n_pol=w.n_pol, b=w.b, row_ptr=w.row_ptr, col_idx=w.col_idx, vals=w.vals)
+    L.dinv = oracle_mg.pbj_invert(L)
+    size = LevelSize(n_brows=L.n_brows, nnzb=L.nnzb, b=L.b)
+    x = np.ascontiguousarray(w.rhs)
+    oracle_mg.spmv(L, x)  # page in
+    reps, t0 = 0, time.perf_counter()
+    while True:
+        y = oracle_mg.spmv(L, x)
+        oracle_mg.pbj_apply(L, y)
+        reps += 1
+        if time.perf_counter() - t0 >= seconds or reps >= 200:
+            break
+    dt = time.perf_counter() - t0
+    gbs = reps * (size.spmv() + size.pbj()) / dt / 1e9
+    threads = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    return gbs, dt, threads, f"{reps} x (block SpMV + PBJ apply) on level 0 of {w.name} ({dt:.1f} s of CPU work)"
+
+
+def orth_bytes(iters, restart, vec_bytes):
+    """CGS2 traffic of ``iters`` Arnoldi steps of GMRES(restart): step j reads V_0..V_j four times (+ w)."""
+    full, rem = divmod(int(iters), int(restart))
+    cyc = sum(4 * (j + 1) + 8 for j in range(restart))
+    return (full * cyc + sum(4 * (j + 1) + 8 for j in range(rem))) * vec_bytes
+
+
+def solve_bytes_from_counts(sizes, outer_iters, coarse_iters, opt):
+    """Algorithmic bytes of one solve from iteration counts alone (used to scale the oracle's GB/s)."""
+    from paper_2506_16676_b200.traffic import vcycle_bytes
+    L0, Lc = sizes[0], sizes[-1]
+    outer = outer_iters * (vcycle_bytes(sizes, opt["nu_pre"], opt["nu_post"]) + L0.spmv()) + \
+        orth_bytes(outer_iters, opt["restart"], L0.vec_bytes)
+    coarse = coarse_iters * (Lc.spmv() + Lc.pbj()) + orth_bytes(coarse_iters, opt["coarse_restart"], Lc.vec_bytes)
+    return outer + coarse
+
+
+def oracle_level_sizes(w):
+    """Level sizes of the hierarchy from the closed-form Galerkin pattern (no numerics): level l+1 has the prism
+    stencil of level l's node graph over min(3, n_phi) planes."""
+    import numpy as np
+    from paper_2506_16676_b200.traffic import LevelSize
+    sizes = [LevelSize(n_brows=w.n_brows, nnzb=w.nnzb, b=w.b)]
+    edges = w.adj_w[0]
+    deg = np.bincount(edges.ravel(), minlength=w.n_pol) + 1   # in-plane blocks per row incl. self
+    n_phi = w.n_phi
+    for _ in range(1, w.levels):
+        n_phi //= 2
+        sizes.append(LevelSize(n_brows=n_phi * w.n_pol, nnzb=int(deg.sum()) * n_phi * min(3, n_phi), b=w.b))
+    return sizes
+
+
+def reference_arm(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_2506_16676_b200.workloads import make_workload
+    from oracle import mg as oracle_mg
+    oracle_mg.build()
+    w = make_workload(args.workload)
+    sizes = oracle_level_sizes(w)
+    opt = dict(nu_pre=2, nu_post=2, restart=100, coarse_restart=50)
+    counts = REFERENCE_COUNTS.get(args.workload, REFERENCE_COUNTS["C1"])
+    total_bytes = solve_bytes_from_counts(sizes, counts["outer_iters"], counts["coarse_iters"], opt)
+    per_step = max(2.0, min(15.0, 150.0 / max(1, args.steps + args.warmup)))
+    for _ in range(args.warmup):
+        oracle_sample(w, per_step)
+    vals, desc, threads = [], "", 1
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        gbs, dt, threads, desc = oracle_sample(w, per_step)
+        vals.append(total_bytes / 1e9 / gbs)
+    wall = time.perf_counter() - t0
+    value = sum(vals) / len(vals)
+    sample = (f"each step: {desc}; measured oracle rate scaled by algorithmic bytes to one solve of "
+              f"{counts['outer_iters']} outer / {counts['coarse_iters']} coarsest-level iterations (counts measured by the "
+              f"CUDA library in round 1; the oracle is not run to convergence at this size)")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * wall / max(1, args.steps), "higher_is_better": False,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "rtol": RTOL, "extrapolated": True},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------- CUDA arm
+def cuda_arm(args):
+    import numpy as np
+    import torch
+    from paper_2506_16676_b200 import binding, buildlib, replicas
+    from paper_2506_16676_b200.workloads import make_workload
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback (use --impl reference for the oracle)")
+    rank, local_rank, world = replicas.init("nccl")
+    if world != args.gpus:
+        log(f"note: --gpus {args.gpus} but WORLD_SIZE {world}; using WORLD_SIZE")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    buildlib.build()
+
+    t0 = time.perf_counter()
+    w = make_workload(args.workload)
+    gen_s = time.perf_counter() - t0
+    rp, ci, va = binding.upload(w, dev)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    s = binding.Solver(rp, ci, va, w.b, w.n_pol, w.n_phi, w.levels)
+    torch.cuda.synchronize()
+    setup_s = time.perf_counter() - t0
+    opt = {k: getattr(s.opt, k) for k in ("nu_pre", "nu_post", "restart", "maxit", "coarse_restart", "coarse_rtol", "coarse_mode")}
+    sizes = level_sizes(s)
+    n = w.n
+    rhs_h = torch.from_numpy(w.rhs.copy()).pin_memory()
+    x_h = torch.empty(n, dtype=torch.float64).pin_memory()
+    if rank == 0:
+        log(f"[bench] workload {w.name}: n = {n}, nnzb = {w.nnzb}, levels = {w.levels}, generate {gen_s:.1f} s, "
+            f"mg_setup {setup_s:.2f} s, hierarchy {s.device_bytes() / 1e9:.2f} GB (+ fine matrix {va.numel() * 8 / 1e9:.2f} GB)")
+
+    info = None
+    for i in range(args.warmup):
+        _, info = s.solve_host(rhs_h, x_h, rtol=RTOL)
+        if rank == 0:
+            log(f"[bench] warm-up {i}: {info['solve_ms'] / 1e3:.2f} s, {info['iters']} its, rel_res {info['rel_res']:.2e}")
+
+    replicas.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    s.profile_reset()
+    launches0 = s.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    dev_ms = 0.0
+    e0.record()
+    for _ in range(args.steps):
+        _, info = s.solve_host(rhs_h, x_h, rtol=RTOL)
+        dev_ms += info["solve_ms"]
+    e1.record()
+    torch.cuda.synchronize()
+    replicas.barrier()
+    e2e_ms = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    launches = s.launch_count() - launches0
+    counts = s.profile_get()
+    if not info["converged"] or not (info["rel_res"] <= 1.05 * RTOL):
+        raise SystemExit(f"bench.py: solve did not reach rtol: {info}")
+    x_dev_check = float(np.abs(x_h.numpy()).max())
+    t_dev = replicas.max_over_ranks(dev_ms / args.steps / 1e3, dev)
+    t_e2e = replicas.max_over_ranks(e2e_ms / args.steps / 1e3, dev)
+
+    # ---- roofline: a short event-bracketed pass (same inputs, a few outer iterations) gives mean kernel durations
+    peak, peak_src = measured_peaks()
+    roof, detail, cpu = None, [], None
+    if rank == 0:
+        s.update_options(maxit=min(opt["maxit"], 2))
+        s.profile_reset()
+        s.profile_enable(True)
+        s.solve_host(rhs_h, x_h, rtol=RTOL)
+        s.profile_enable(False)
+        timed = s.profile_get()
+        s.update_options(maxit=opt["maxit"])
+        restart_by_level = {s.levels - 1: opt["coarse_restart"]}
+        step_ms_model = 0.0
+        for (level, kind), c in counts.items():
+            t = timed.get((level, kind))
+            if not t or not t["timed"]:
+                continue
+            mean_ms = t["ms"] / t["timed"]
+            per_step_launches = c["launches"] / args.steps
+            nbytes = class_bytes(sizes, level, kind, restart_by_level)
+            share_ms = per_step_launches * mean_ms
+            step_ms_model += share_ms
+            detail.append({"level": level, "kind": kind, "launches_per_step": per_step_launches, "mean_us": 1e3 * mean_ms,
+                           "bytes_per_launch": nbytes, "GBps": (nbytes / mean_ms / 1e6) if nbytes else None,
+                           "frac": (nbytes / mean_ms / 1e6 / peak) if nbytes else None, "ms_per_step": share_ms})
+        detail.sort(key=lambda d: -d["ms_per_step"])
+        for d in detail:
+            d["share_of_step"] = d["ms_per_step"] / (1e3 * t_dev)
+        top = next((d for d in detail if d["bytes_per_launch"]), None)
+        if top:
+            roof = {"bound": "hbm", "kernel": f"bsr kernel, kind {top['kind']}, level {top['level']}", "achieved": top["GBps"],
+                    "peak": peak, "unit": "GB/s", "frac": top["frac"], "traffic": None, "peak_source": peak_src,
+                    "bytes_per_launch": top["bytes_per_launch"], "mean_us": top["mean_us"],
+                    "share_of_step": top["share_of_step"], "frac_of_8TBs_nominal": top["GBps"] / 8000.0}
+        # ---- oracle timed beside it (rank 0, N = 1 only)
+        if world == 1 and not args.no_cpu_baseline:
+            gbs, dt, threads, desc = oracle_sample(w, args.cpu_seconds)
+            total_bytes = sum(c["launches"] / args.steps * class_bytes(sizes, level, kind, restart_by_level)
+                              for (level, kind), c in counts.items())
+            # orthogonalisation launches carry no per-launch size: their traffic follows from the iteration counts
+            total_bytes += orth_bytes(info["iters"], opt["restart"], sizes[0].vec_bytes)
+            if not any(kind == "cycle" for (_, kind) in counts):
+                total_bytes += orth_bytes(info["coarse_iters_total"], opt["coarse_restart"], sizes[-1].vec_bytes)
+            cpu = {"value": total_bytes / 1e9 / gbs, "unit": UNIT, "cores": threads, "kind": "oracle",
+                   "oracle_GBps": gbs,
+                   "sample": f"{desc}; its algorithmic GB/s scaled to the {total_bytes / 1e9:.0f} GB of algorithmic "
+                             f"traffic of one solve ({info['iters']} outer, {info['coarse_iters_total']} coarsest-level iterations)"}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": t_dev, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": 1e3 * t_dev, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic",
+                "config": {"workload": w.name, "n_pol": w.n_pol, "n_phi": w.n_phi, "b": w.b, "levels": w.levels,
+                           "unknowns": n, "nnzb": w.nnzb, "rtol": RTOL, "cycle": f"V({opt['nu_pre']},{opt['nu_post']}) PBJ-Chebyshev",
+                           "coarsest": f"PBJ-GMRES({opt['coarse_restart']}) to {opt['coarse_rtol']:g}", "fgmres_restart": opt["restart"],
+                           "parallelism": "replicas only" if world > 1 else "1 GPU", "setup_s": setup_s,
+                           "l2": "inputs larger than L2 (every level's matrix >= 0.5 GB vs 126 MB L2)" if sizes[-1].matrix_bytes > 2.6e8
+                           else "coarsest level fits L2: not an HBM-roofline workload",
+                           "outer_iters": info["iters"], "coarse_iters": info["coarse_iters_total"], "rel_res": info["rel_res"],
+                           "max_abs_x": x_dev_check},
+                "e2e": {"value": t_e2e, "unit": UNIT, "h2d_bytes_per_step": 8 * n, "d2h_bytes_per_step": 8 * n},
+                "gpu_launches": launches, "clocks": clocks, "roofline": roof, "cpu_baseline": cpu,
+                "throughput": {"value": world / t_dev, "unit": "solves/s"},
+                "kernels": detail[:12]}
+        print(json.dumps(line), flush=True)
+    s.destroy()
+    replicas.finalize()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=1)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
+    ap.add_argument("--workload", default="C1", help="C1 (the metric's config, default); C0, C2-16/32/64, C3 for other configs")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="CPU time of the oracle sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.steps < 1 or args.warmup < 0:
+        ap.error("--steps >= 1 and --warmup >= 0")
+    return reference_arm(args) if args.impl == "reference" else cuda_arm(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

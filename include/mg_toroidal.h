@@ -78,6 +78,7 @@ typedef struct mg_options {
 typedef struct mg_solve_info {
     int iters;              /* outer FGMRES iterations = number of V-cycle applications */
     int converged;          /* 1 if the Arnoldi residual estimate reached rtol*|b| */
+    double solve_ms;        /* device time of the solve (CUDA events on the stream, inputs resident in HBM) */
     double rel_res;         /* true |b - A x| / |b| recomputed after the solve */
     int coarse_iters_total; /* coarsest-level GMRES iterations summed over all V-cycles */
     int hist_len;           /* in: capacity of hist; out: entries written (iters + 1, clipped) */
@@ -148,6 +149,27 @@ int mg_copy_level_to_host(mg_handle *h, int level, int64_t *row_ptr_host, int32_
                           double *dinv_host);
 /* Override the Chebyshev interval of one level (parity tests inject the oracle's bounds). */
 int mg_set_cheb_bounds(mg_handle *h, int level, double lam_min, double lam_max);
+/* ---- profiling: per-(level, kind) device time of the library's own kernel launches --------------------- */
+#define MG_KIND_SPMV 0      /* y = A x */
+#define MG_KIND_RESID 1     /* r = rhs - A x */
+#define MG_KIND_SWEEP 2     /* fused PBJ-Chebyshev sweep: r -= A d, z = D^-1 r, d' = c_d d + c_z z, x update */
+#define MG_KIND_SWEEP_NOD 3 /* last pre-smoothing sweep: r -= A d, x += d (no D^-1 pass) */
+#define MG_KIND_PBJ 4       /* z = D^-1 r */
+#define MG_KIND_RESTRICT 5
+#define MG_KIND_PROLONG 6
+#define MG_KIND_ORTH 7      /* (F)GMRES dots / axpys / Givens bookkeeping */
+#define MG_KIND_OTHER 8
+#define MG_KIND_CYCLE 9     /* one whole coarsest-level GMRES restart cycle in a single persistent kernel */
+#define MG_KIND_COUNT 10
+#define MG_PROFILE_MAX_LEVELS 32
+/* Launches are always counted per (level, kind).  on != 0 additionally brackets every kernel launch with a
+ * CUDA event pair on the stream and books its duration; CUDA-graph replay is bypassed while that is on. */
+int mg_profile_enable(mg_handle *h, int on);
+int mg_profile_reset(mg_handle *h);
+/* One (level, kind) class since the last reset: launches (all), timed (launches that were event-bracketed)
+ * and ms (their summed device milliseconds).  Any out pointer may be NULL.  Synchronises the stream. */
+int mg_profile_get(mg_handle *h, int level, int kind, int64_t *launches, int64_t *timed, double *ms);
+
 /* Number of CUDA kernels this handle has launched so far (graph replays count their kernel nodes). */
 int64_t mg_launch_count(mg_handle *h);
 /* Bytes of device memory the handle has allocated. */

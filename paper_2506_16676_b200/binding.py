@@ -13,6 +13,7 @@ import os
 from . import buildlib
 
 MG_OK, MG_EINVAL, MG_ENOMEM, MG_ESINGULAR, MG_ECUDA = 0, -1, -2, -3, -4
+KIND_NAMES = ("spmv", "resid", "sweep", "sweep_nod", "pbj", "restrict", "prolong", "orth", "other", "cycle")
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
 FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
@@ -27,7 +28,7 @@ class mg_options(C.Structure):
 
 
 class mg_solve_info(C.Structure):
-    _fields_ = [("iters", C.c_int), ("converged", C.c_int), ("rel_res", C.c_double), ("coarse_iters_total", C.c_int),
+    _fields_ = [("iters", C.c_int), ("converged", C.c_int), ("solve_ms", C.c_double), ("rel_res", C.c_double), ("coarse_iters_total", C.c_int),
                 ("hist_len", C.c_int), ("hist", C.POINTER(C.c_double))]
 
 
@@ -52,6 +53,9 @@ SYMBOLS = {
                           C.POINTER(_VP), C.POINTER(_D), C.POINTER(_D), C.POINTER(_D)]),
     "mg_copy_level_to_host": (_I, [_VP, _I, _VP, _VP, _VP, _VP]),
     "mg_set_cheb_bounds": (_I, [_VP, _I, _D, _D]),
+    "mg_profile_enable": (_I, [_VP, _I]),
+    "mg_profile_reset": (_I, [_VP]),
+    "mg_profile_get": (_I, [_VP, _I, _I, C.POINTER(_I64), C.POINTER(_I64), C.POINTER(_D)]),
     "mg_launch_count": (_I64, [_VP]),
     "mg_device_bytes": (_I64, [_VP]),
     "mg_strerror": (C.c_char_p, [_I]),
@@ -268,6 +272,24 @@ class Solver:
     def set_cheb_bounds(self, level, lam_min, lam_max):
         _chk(lib().mg_set_cheb_bounds(self._h, level, float(lam_min), float(lam_max)), "mg_set_cheb_bounds")
 
+    def profile_enable(self, on: bool = True):
+        _chk(lib().mg_profile_enable(self._h, int(bool(on))), "mg_profile_enable")
+
+    def profile_reset(self):
+        _chk(lib().mg_profile_reset(self._h), "mg_profile_reset")
+
+    def profile_get(self) -> dict:
+        """{(level, kind_name): dict(launches, timed, ms)} of every class that launched since the last reset."""
+        out = {}
+        for level in range(self.levels):
+            for kind, name in enumerate(KIND_NAMES):
+                n, nt, ms = C.c_int64(), C.c_int64(), C.c_double()
+                _chk(lib().mg_profile_get(self._h, level, kind, C.byref(n), C.byref(nt), C.byref(ms)),
+                     "mg_profile_get")
+                if n.value:
+                    out[(level, name)] = dict(launches=n.value, timed=nt.value, ms=ms.value)
+        return out
+
     def launch_count(self) -> int:
         return int(lib().mg_launch_count(self._h))
 
@@ -276,7 +298,7 @@ class Solver:
 
 
 def _info_dict(info, hist):
-    return dict(iters=info.iters, converged=bool(info.converged), rel_res=info.rel_res,
+    return dict(iters=info.iters, converged=bool(info.converged), solve_ms=info.solve_ms, rel_res=info.rel_res,
                 coarse_iters_total=info.coarse_iters_total,
                 hist=[hist[i] for i in range(info.hist_len)] if hist is not None else [])
 

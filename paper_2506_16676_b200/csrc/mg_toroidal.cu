@@ -22,6 +22,7 @@ namespace {
 thread_local std::string g_last_cuda_error;
 
 struct Level {
+    int index = 0;
     int n_phi = 0;
     int64_t n_brows = 0, nnzb = 0, nvec = 0;
     const int64_t *row_ptr = nullptr;
@@ -35,6 +36,16 @@ struct Level {
     std::vector<int32_t> h_col_idx;
 };
 
+struct ProfPair {
+    cudaEvent_t e0, e1;
+    int level, kind;
+};
+struct ProfAcc {
+    int64_t launches = 0;  // every launch since the last reset (graph replays included)
+    int64_t timed = 0;     // launches bracketed by events while profiling was on
+    double ms = 0.0;       // their summed device time
+};
+
 struct Gmres {
     GmresDev dev{};
     int m = 0, maxit = 0;
@@ -45,6 +56,7 @@ struct Gmres {
     int red_grid = 0;
     bool flexible = false;
     bool ready = false;
+    int level = 0;  // level whose vectors this engine orthogonalises (profiling only)
 };
 
 }  // namespace
@@ -70,6 +82,14 @@ struct mg_handle {
     int64_t capture_count = 0;
     double *d_rhs_host = nullptr, *d_x_host = nullptr;  // device staging for mg_solve_host
     int coarse_iters_total = 0, coarse_iters_last = 0;
+    cudaEvent_t ev_solve[2] = {nullptr, nullptr};        // device time of the last mg_solve
+    // profiling (mg_profile_enable): every launch is bracketed by an event pair and booked per (level, kind)
+    bool profiling = false;
+    int cur_level = 0, cur_kind = MG_KIND_OTHER;
+    std::vector<ProfPair> prof_pending;
+    std::vector<cudaEvent_t> prof_free;
+    ProfAcc prof[MG_PROFILE_MAX_LEVELS][MG_KIND_COUNT];
+    int64_t graph_hist[MG_PROFILE_MAX_LEVELS][MG_KIND_COUNT] = {};  // kernel nodes of the captured coarse cycle
 };
 
 namespace {
@@ -90,14 +110,76 @@ int cuda_fail(cudaError_t e, const char *what) {
     } while (0)
 
 inline void count_launch(mg_handle *h) {
-    if (h->capturing) h->capture_count++;
-    else h->launches++;
+    const int lv = std::min(h->cur_level, MG_PROFILE_MAX_LEVELS - 1);
+    if (h->capturing) {
+        h->capture_count++;
+        h->graph_hist[lv][h->cur_kind]++;
+    } else {
+        h->launches++;
+        h->prof[lv][h->cur_kind].launches++;
+    }
+}
+
+// Profiling: resolve the pending event pairs into the per-(level, kind) accumulators (synchronises the stream).
+void prof_flush(mg_handle *h) {
+    if (h->prof_pending.empty()) return;
+    cudaStreamSynchronize(h->stream);
+    for (const ProfPair &pp : h->prof_pending) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, pp.e0, pp.e1) == cudaSuccess) {
+            ProfAcc &a = h->prof[std::min(pp.level, MG_PROFILE_MAX_LEVELS - 1)][pp.kind];
+            a.timed++;
+            a.ms += ms;
+        }
+        h->prof_free.push_back(pp.e0);
+        h->prof_free.push_back(pp.e1);
+    }
+    h->prof_pending.clear();
+}
+inline cudaEvent_t prof_event(mg_handle *h) {
+    if (!h->prof_free.empty()) {
+        cudaEvent_t e = h->prof_free.back();
+        h->prof_free.pop_back();
+        return e;
+    }
+    cudaEvent_t e = nullptr;
+    cudaEventCreate(&e);
+    return e;
+}
+inline bool prof_begin(mg_handle *h, ProfPair &pp) {
+    if (!h->profiling || h->capturing) return false;
+    if (h->prof_pending.size() >= 2048) prof_flush(h);
+    pp.e0 = prof_event(h);
+    pp.e1 = prof_event(h);
+    pp.level = h->cur_level;
+    pp.kind = h->cur_kind;
+    cudaEventRecord(pp.e0, h->stream);
+    return true;
+}
+inline void prof_end(mg_handle *h, ProfPair &pp) {
+    cudaEventRecord(pp.e1, h->stream);
+    h->prof_pending.push_back(pp);
 }
 #define LAUNCH(h, kern, grid, block, smem, ...)                     \
     do {                                                            \
+        ProfPair pp__;                                              \
+        const bool prof__ = prof_begin(h, pp__);                    \
         kern<<<(grid), (block), (smem), (h)->stream>>>(__VA_ARGS__); \
+        if (prof__) prof_end(h, pp__);                              \
         count_launch(h);                                            \
     } while (0)
+struct KindScope {  // books the launches of one scope under (level, kind)
+    mg_handle *h;
+    int level0, kind0;
+    KindScope(mg_handle *hh, int level, int kind) : h(hh), level0(hh->cur_level), kind0(hh->cur_kind) {
+        h->cur_level = level;
+        h->cur_kind = kind;
+    }
+    ~KindScope() {
+        h->cur_level = level0;
+        h->cur_kind = kind0;
+    }
+};
 
 int dalloc(mg_handle *h, void **p, size_t bytes) {
     bytes = std::max<size_t>(bytes, 16);
@@ -135,6 +217,9 @@ int launch_bsr(mg_handle *h, const Level &L, BsrArgs a) {
     a.dinv = L.dinv;
     a.n_brows = L.n_brows;
     if (L.n_brows == 0) return MG_OK;
+    const int kind = a.mode == MODE_SPMV ? MG_KIND_SPMV : a.mode == MODE_RESID ? MG_KIND_RESID : a.mode == MODE_PBJ ? MG_KIND_PBJ
+                     : (a.flags & F_NEED_D) ? MG_KIND_SWEEP : MG_KIND_SWEEP_NOD;
+    KindScope scope(h, L.index, kind);
     switch (h->b) {
 #define BSR_CASE(B)                                                                                          \
     case B: {                                                                                                \
@@ -275,6 +360,7 @@ int postsmooth(mg_handle *h, Level &L, const double *v, double *x, int nu) {
 int restrict_to(mg_handle *h, int l, const double *rf, double *rc) {
     const Level &L = h->lev[l];
     const int64_t plane = (int64_t)h->n_pol * h->b;
+    KindScope scope(h, l, MG_KIND_RESTRICT);
     LAUNCH(h, restrict_kernel, grid_for(plane * (L.n_phi / 2), 256), 256, 0, rf, rc, plane, L.n_phi, (const int *)nullptr);
     CU(cudaGetLastError());
     return MG_OK;
@@ -282,6 +368,7 @@ int restrict_to(mg_handle *h, int l, const double *rf, double *rc) {
 int prolong_add(mg_handle *h, int l, const double *ec, double *xf, double *pe) {
     const Level &L = h->lev[l];
     const int64_t plane = (int64_t)h->n_pol * h->b;
+    KindScope scope(h, l, MG_KIND_PROLONG);
     LAUNCH(h, prolong_add_kernel, grid_for(plane * L.n_phi, 256), 256, 0, ec, xf, pe, plane, L.n_phi, (const int *)nullptr);
     CU(cudaGetLastError());
     return MG_OK;
@@ -323,6 +410,7 @@ int gmres_alloc(mg_handle *h, Gmres &G, int64_t n, int m, int maxit, bool flexib
 
 // tol = rtol * ||rhs||, iteration counters reset.
 int gmres_start(mg_handle *h, Gmres &G, const double *rhs, double rtol) {
+    KindScope scope(h, G.level, MG_KIND_ORTH);
     LAUNCH(h, dot_multi_kernel, dim3(G.red_grid, 1), 256, 0, rhs, (int64_t)0, rhs, G.n, G.partial, G.counter,
            G.dev.nrm2, (const int *)nullptr);
     LAUNCH(h, gmres_set_tol_kernel, 1, 1, 0, G.dev, rtol);
@@ -331,6 +419,7 @@ int gmres_start(mg_handle *h, Gmres &G, const double *rhs, double rtol) {
 }
 // V[0] holds the residual r: beta = ||r||, stop test, g = beta e_1, V[0] /= beta.
 int gmres_cycle_begin(mg_handle *h, Gmres &G) {
+    KindScope scope(h, G.level, MG_KIND_ORTH);
     const int *done = G.dev.status;
     LAUNCH(h, dot_multi_kernel, dim3(G.red_grid, 1), 256, 0, G.V, (int64_t)0, G.V, G.n, G.partial, G.counter, G.dev.nrm2,
            done);
@@ -340,6 +429,7 @@ int gmres_cycle_begin(mg_handle *h, Gmres &G) {
 }
 // V[j+1] holds w = A M v_j: two classical Gram-Schmidt passes against V[0..j], Hessenberg column, v_{j+1}.
 int gmres_orth(mg_handle *h, Gmres &G, int j) {
+    KindScope scope(h, G.level, MG_KIND_ORTH);
     const int *done = G.dev.status;
     double *w = G.V + (size_t)(j + 1) * G.stride;
     const int axpy_grid = (int)((G.n / 2 + 256) / 256);
@@ -357,6 +447,7 @@ int gmres_orth(mg_handle *h, Gmres &G, int j) {
 }
 // y = H^-1 g ; out += sum_i y_i B_i  (B = Z for flexible, V otherwise)
 int gmres_cycle_end(mg_handle *h, Gmres &G, double *out) {
+    KindScope scope(h, G.level, MG_KIND_ORTH);
     LAUNCH(h, gmres_solve_y_kernel, 1, 1, 0, G.dev);
     const int axpy_grid = (int)((G.n / 2 + 256) / 256);
     LAUNCH(h, axpy_multi_kernel, axpy_grid, 256, 0, G.flexible ? G.Z : G.V, G.stride, G.m, G.dev.status + 1, G.dev.y, 1.0,
@@ -404,10 +495,12 @@ int coarse_solve_internal(mg_handle *h) {
             h->coarse_graph = nullptr;
         }
         MG(gmres_alloc(h, G, L.nvec, h->opt.coarse_restart, h->opt.coarse_maxit, false));
+        G.level = L.index;
     }
     CU(cudaMemsetAsync(L.x, 0, (size_t)L.nvec * sizeof(double), h->stream));
     MG(gmres_start(h, G, L.rhs, h->opt.coarse_rtol));
-    if (h->opt.use_graphs && !h->coarse_graph) {
+    const bool use_graph = h->opt.use_graphs && !h->profiling;
+    if (use_graph && !h->coarse_graph) {
         cudaGraph_t graph = nullptr;
         if (!h->cap_stream) CU(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
         cudaStream_t user_stream = h->stream;
@@ -415,6 +508,7 @@ int coarse_solve_internal(mg_handle *h) {
         h->stream = h->cap_stream;
         h->capturing = true;
         h->capture_count = 0;
+        std::memset(h->graph_hist, 0, sizeof(h->graph_hist));
         const int rc = coarse_cycle_enqueue(h);
         h->capturing = false;
         h->stream = user_stream;
@@ -431,9 +525,11 @@ int coarse_solve_internal(mg_handle *h) {
     }
     int st[4] = {0, 0, 0, 0};
     do {
-        if (h->coarse_graph) {
+        if (use_graph) {
             CU(cudaGraphLaunch(h->coarse_graph, h->stream));
             h->launches += h->coarse_graph_kernels;
+            for (int lv = 0; lv < MG_PROFILE_MAX_LEVELS; ++lv)
+                for (int k = 0; k < MG_KIND_COUNT; ++k) h->prof[lv][k].launches += h->graph_hist[lv][k];
         } else {
             MG(coarse_cycle_enqueue(h));
         }
@@ -664,6 +760,13 @@ int mg_destroy(mg_handle *h) {
     cudaStreamSynchronize(h->stream);
     if (h->coarse_graph) cudaGraphExecDestroy(h->coarse_graph);
     if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+    for (const ProfPair &pp : h->prof_pending) {
+        cudaEventDestroy(pp.e0);
+        cudaEventDestroy(pp.e1);
+    }
+    for (cudaEvent_t e : h->prof_free) cudaEventDestroy(e);
+    for (cudaEvent_t e : h->ev_solve)
+        if (e) cudaEventDestroy(e);
     for (void *p : h->owned) {
         if (h->opt.free) h->opt.free(p, h->opt.alloc_ctx);
         else if (!h->opt.alloc) cudaFree(p);
@@ -698,6 +801,7 @@ int mg_setup(mg_handle **out, const int64_t *row_ptr, const int32_t *col_idx, co
     h->n_levels = levels;
     h->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
     h->lev.resize(levels);
+    for (int l = 0; l < levels; ++l) h->lev[l].index = l;
     int rc = MG_OK;
     auto fail = [&](int code) {
         mg_destroy(h);
@@ -769,6 +873,11 @@ int mg_solve(mg_handle *h, const double *rhs, double *x, double rtol, int x_is_i
     if (!G.ready || G.m != h->opt.restart || G.maxit != h->opt.maxit)
         MG(gmres_alloc(h, G, n, h->opt.restart, h->opt.maxit, true));
     h->coarse_iters_total = 0;
+    if (!h->ev_solve[0]) {
+        CU(cudaEventCreate(&h->ev_solve[0]));
+        CU(cudaEventCreate(&h->ev_solve[1]));
+    }
+    CU(cudaEventRecord(h->ev_solve[0], h->stream));
     if (!x_is_initial_guess) CU(cudaMemsetAsync(x, 0, bytes, h->stream));
     MG(gmres_start(h, G, rhs, rtol));
     CU(cudaMemcpyAsync(h->pinned_d, G.dev.nrm2, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
@@ -781,6 +890,7 @@ int mg_solve(mg_handle *h, const double *rhs, double *x, double rtol, int x_is_i
         if (info) {
             info->iters = 0;
             info->converged = 1;
+            info->solve_ms = 0.0;
             info->rel_res = 0.0;
             info->coarse_iters_total = 0;
             if (info->hist && info->hist_len > 0) info->hist[0] = 0.0;
@@ -808,7 +918,12 @@ int mg_solve(mg_handle *h, const double *rhs, double *x, double rtol, int x_is_i
     MG(residual(h, L, rhs, x, L.r));
     double rn2 = 0.0;
     MG(dot_host(h, L.r, L.r, n, &rn2));
+    CU(cudaEventRecord(h->ev_solve[1], h->stream));
+    CU(cudaEventSynchronize(h->ev_solve[1]));
+    float solve_ms = 0.f;
+    CU(cudaEventElapsedTime(&solve_ms, h->ev_solve[0], h->ev_solve[1]));
     if (info) {
+        info->solve_ms = solve_ms;
         info->iters = st[2];
         info->converged = st[3];
         info->rel_res = std::sqrt(std::max(rn2, 0.0)) / bnorm;
@@ -927,6 +1042,30 @@ int mg_set_cheb_bounds(mg_handle *h, int level, double lam_min, double lam_max) 
     if (!level_ok(h, level) || !(lam_min > 0.0) || !(lam_max > lam_min)) return MG_EINVAL;
     h->lev[level].lam_min = lam_min;
     h->lev[level].lam_max = lam_max;
+    return MG_OK;
+}
+
+int mg_profile_enable(mg_handle *h, int on) {
+    if (!h) return MG_EINVAL;
+    prof_flush(h);
+    h->profiling = (on != 0);
+    return MG_OK;
+}
+
+int mg_profile_reset(mg_handle *h) {
+    if (!h) return MG_EINVAL;
+    prof_flush(h);
+    for (auto &row : h->prof)
+        for (auto &a : row) a = ProfAcc();
+    return MG_OK;
+}
+
+int mg_profile_get(mg_handle *h, int level, int kind, int64_t *launches, int64_t *timed, double *ms) {
+    if (!h || level < 0 || level >= MG_PROFILE_MAX_LEVELS || kind < 0 || kind >= MG_KIND_COUNT) return MG_EINVAL;
+    prof_flush(h);
+    if (launches) *launches = h->prof[level][kind].launches;
+    if (timed) *timed = h->prof[level][kind].timed;
+    if (ms) *ms = h->prof[level][kind].ms;
     return MG_OK;
 }
 
