@@ -361,6 +361,22 @@ def cuda_arm(args):
     return 0
 
 
+def kernel_sweep_arm(args):
+    """configs[4] "Kernel sweep for the roofline": GB/s and fraction of the HBM peak per point."""
+    import torch
+    from paper_2506_16676_b200 import buildlib, kernel_sweep
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(0)
+    buildlib.build()
+    peak, peak_src = measured_peaks()
+    for rep in kernel_sweep.run(peak, points=args.kernel_sweep or None, reps=max(3, args.steps),
+                                shuffled=args.sweep_shuffled, max_gb=args.sweep_max_gb):
+        rep.update(peak_GBps=peak, peak_source=peak_src, dtype="f64", data="synthetic")
+        print(json.dumps(rep), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     ap.add_argument("--gpus", type=int, default=1)
@@ -373,7 +389,14 @@ def main():
     ap.add_argument("--max-outer", type=int, default=0,
                     help="profiling aid (ncu launch lists): cap the outer FGMRES iterations of every solve; the line is then "
                          "marked \"truncated\": true and is NOT a bench value")
+    ap.add_argument("--kernel-sweep", nargs="*", default=None, metavar="TOKEN",
+                    help="configs[4]: time the block SpMV and one PBJ-Chebyshev sweep on the C4 points (all, or those whose "
+                         "name contains a TOKEN, e.g. b36 n2000-p16) and print one JSON line per point instead of the solve line")
+    ap.add_argument("--sweep-max-gb", type=float, default=50.0, help="skip C4 points whose matrix exceeds this size")
+    ap.add_argument("--sweep-shuffled", action="store_true", help="C4 'shuffled' variant: permuted node numbering")
     args = ap.parse_args()
+    if args.kernel_sweep is not None:
+        return kernel_sweep_arm(args)
     if args.steps < 1 or args.warmup < 0:
         ap.error("--steps >= 1 and --warmup >= 0")
     return reference_arm(args) if args.impl == "reference" else cuda_arm(args)
