@@ -70,6 +70,9 @@ typedef struct mg_options {
                                 (paper: 200 / 200) */
     int block_layout;        /* 0: row-major b x b blocks (only layout supported) */
     int use_graphs;          /* 1 (default): the coarse GMRES restart cycle is replayed as a CUDA graph */
+    int kernel_variant;      /* launch mechanics only (same arithmetic up to summation order): 0 (default) the
+                                persistent TMA-ring block-CSR kernel where it exists (b = 36), 1 the one-CTA-per-row
+                                128-bit-load kernel for every b (kept for A/B measurement) */
     mg_alloc_fn alloc;       /* NULL => cudaMalloc */
     mg_free_fn free;         /* NULL => cudaFree */
     void *alloc_ctx;

@@ -1,0 +1,322 @@
+// kernels_bsr_tma.cuh -- block-CSR kernels of the solve path for b = 36 on sm_100a: SpMV, residual, PBJ apply
+// and the fused PBJ-Chebyshev sweep as ONE persistent kernel whose
+// matrix stream is moved by the TMA engine.
+//
+// Why: every step is a scan with 0.25 flop/byte, so the only thing that matters is keeping HBM busy.  The first
+// kernel of this library (kernels_bsr.cuh: one CTA per block row, 128-bit loads into registers) moved exactly the
+// algorithmic bytes but was latency bound at 72 % of the measured copy rate (profiles/r01_baseline_ldg_kernel.md:
+// 2 CTAs per SM, every CTA drains its loads before it reduces).  Here loading and arithmetic are decoupled:
+//
+//   * grid = one persistent CTA per SM; CTA k owns a CONTIGUOUS range of block rows holding ~nnzb/grid blocks
+//     (partition table built in mg_setup), hence one contiguous span of `vals`;
+//   * a producer warp streams that span block by block (b*b*8 = 10,368 B) with 1-D bulk async copies
+//     (cp.async.bulk -> SASS UBLKCP) into a ring of STAGES shared-memory stages, and with each block the x_J it
+//     multiplies (288 B, an L2 hit), both completing on the stage's "full" mbarrier.  STAGES * 10.6 KB ~ 213 KB are
+//     in flight per SM whatever the consumers do;
+//   * NG consumer groups of 160 threads take the CTA's rows round-robin.  Thread t < 144 of a group owns the
+//     9-element segment [9t, 9t+9) of every block of its row (row t/4, columns 9(t%4)..): shared-memory reads at a
+//     9-double stride are bank-conflict free, the 4 partial sums of a row meet by two warp shuffles, blocks are
+//     added in stored order (deterministic).  After the last read of a stage each consumer warp arrives on the
+//     stage's "empty" mbarrier, which hands it back to the producer;
+//   * the row epilogue is the fused part: residual, x update, z = Dinv_I r_I (Dinv_I prefetched into registers at
+//     row start, 9 doubles per thread), Chebyshev direction update -- kernels_bsr.cuh documents the modes.
+//
+// PBJ apply alone is the same kernel on the implicit block-diagonal matrix `dinv` (row I = block I = column I).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "kernels_bsr.cuh"
+
+namespace mgk {
+
+struct TmaCfg {
+    static constexpr int B = 36, BB = B * B;
+    static constexpr int SEGL = 9;                    // segment length (doubles) owned by one thread
+    static constexpr int SEG = B / SEGL;              // 4 segments per block row
+    static constexpr int ACTIVE = B * SEG;            // 144 working threads per group
+    static constexpr int GROUP = 160;                 // 5 warps per group (16 idle lanes)
+    static constexpr int GWARPS = GROUP / 32;
+    static constexpr int NG = 4;                      // consumer groups per CTA
+    static constexpr int STAGES = 20;
+    static constexpr int THREADS = NG * GROUP + 32;   // + 1 producer warp
+    static constexpr int VECPAD = 40;
+    static constexpr size_t SMEM = sizeof(double) * ((size_t)STAGES * (BB + B) + NG * VECPAD) + sizeof(uint64_t) * (2 * STAGES + 2);
+};
+
+// extra arguments of the TMA kernel (the common ones are BsrArgs)
+struct TmaExtra {
+    const int64_t *part;      // [gridDim.x + 1] first block row of every CTA (nullptr: uniform split, implicit diagonal)
+    const double *scale_div;  // PBJ mode, optional: the input is rin / *scale_div
+    double *vout;             // PBJ mode, optional: vout_I = rin_I / *scale_div
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+    uint32_t ok;
+    do {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n"
+            : "=r"(ok)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+    } while (!ok);
+}
+// 1-D bulk async copy global -> shared, completing `bytes` on the mbarrier (TMA engine; SASS UBLKCP).
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_g2s_hint(void *dst, const void *src, uint32_t bytes, uint64_t *bar, uint64_t policy) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+            smem_u32(dst)),
+        "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
+        : "memory");
+}
+__device__ __forceinline__ uint64_t policy_evict_first() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void group_bar(int g) {
+    asm volatile("bar.sync %0, %1;" ::"r"(g + 1), "n"(TmaCfg::GROUP) : "memory");
+}
+
+// part[k] = first block row I with row_ptr[I] >= k * nnzb / nparts (k = 0..nparts; part[nparts] = n_brows):
+// contiguous row ranges holding (nearly) equal numbers of blocks.
+__global__ void partition_rows_kernel(const int64_t *__restrict__ row_ptr, const int64_t n_brows, const int64_t nnzb,
+                                      const int nparts, int64_t *__restrict__ part) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k > nparts) return;
+    if (k == nparts) {
+        part[k] = n_brows;
+        return;
+    }
+    const int64_t target = (int64_t)(((__int128)nnzb * k) / nparts);
+    int64_t lo = 0, hi = n_brows;  // first I in [0, n_brows] with row_ptr[I] >= target
+    while (lo < hi) {
+        const int64_t mid = (lo + hi) >> 1;
+        if (row_ptr[mid] >= target) hi = mid; else lo = mid + 1;
+    }
+    part[k] = lo;
+}
+
+__global__ void __launch_bounds__(TmaCfg::THREADS, 1) bsr_tma_kernel(const BsrArgs a, const TmaExtra ex) {
+    using C = TmaCfg;
+    constexpr int B = C::B, BB = C::BB;
+    if (a.done != nullptr && *a.done != 0) return;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double *sA = reinterpret_cast<double *>(smem_raw);
+    double *sX = sA + (size_t)C::STAGES * BB;
+    double *sVec = sX + C::STAGES * B;
+    uint64_t *full = reinterpret_cast<uint64_t *>(sVec + C::NG * C::VECPAD);
+    uint64_t *empty = full + C::STAGES;
+    // number of blocks the producer has issued so far.  A consumer group may be more than one ring round ahead of
+    // the stage it wants next (its row starts >= STAGES blocks after the oldest block still in flight); an
+    // mbarrier parity wait is only meaningful for the current or the preceding phase, so the group first waits
+    // until its block has been ISSUED (then the stage's previous round is consumed and its phase is the current one).
+    volatile int *issued = reinterpret_cast<volatile int *>(empty + C::STAGES);
+
+    const bool diag = (a.mode == MODE_PBJ);             // implicit block-diagonal matrix `dinv`, x block = rin_I
+    const double *stream = diag ? a.dinv : a.vals;
+    const double *xsrc = diag ? a.rin : a.vin;
+    int64_t R0, R1;
+    if (ex.part != nullptr) {
+        R0 = ex.part[blockIdx.x];
+        R1 = ex.part[blockIdx.x + 1];
+    } else {
+        R0 = a.n_brows * blockIdx.x / gridDim.x;
+        R1 = a.n_brows * (blockIdx.x + 1) / gridDim.x;
+    }
+    if (R0 >= R1) return;
+    const int64_t P0 = diag ? R0 : a.row_ptr[R0];
+    const int64_t P1 = diag ? R1 : a.row_ptr[R1];
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) {
+        *issued = 0;
+        for (int s = 0; s < C::STAGES; ++s) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], C::GWARPS);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (warp == C::NG * C::GWARPS) {
+        // ------------------------------------------------------------------ producer warp: stream blocks P0..P1
+        const uint64_t pol = policy_evict_first();
+        const int total = (int)(P1 - P0);
+        int cnext = 0;
+        if (lane < total) cnext = diag ? (int)(P0 + lane) : __ldg(a.col_idx + P0 + lane);
+        int s = 0;
+        uint32_t ph = 0;
+        for (int base = 0; base < total; base += 32) {
+            const int c = cnext;
+            const int nb = base + 32 + lane;
+            if (nb < total) cnext = diag ? (int)(P0 + nb) : __ldg(a.col_idx + P0 + nb);
+            const int cnt = min(32, total - base);
+            for (int i = 0; i < cnt; ++i) {
+                const int j = __shfl_sync(0xffffffffu, c, i);
+                if (lane == 0) {
+                    mbar_wait(&empty[s], ph ^ 1u);
+                    mbar_expect_tx(&full[s], (uint32_t)((BB + B) * sizeof(double)));
+                    bulk_g2s_hint(sA + (size_t)s * BB, stream + (size_t)(P0 + base + i) * BB, BB * sizeof(double), &full[s], pol);
+                    bulk_g2s(sX + s * B, xsrc + (size_t)j * B, B * sizeof(double), &full[s]);
+                    __threadfence_block();
+                    *issued = base + i + 1;
+                }
+                if (++s == C::STAGES) {
+                    s = 0;
+                    ph ^= 1u;
+                }
+            }
+        }
+        return;
+    }
+
+    // ---------------------------------------------------------------------- consumer groups: rows R0+g, R0+g+NG, ...
+    const int g = tid / C::GROUP, t = tid - g * C::GROUP;
+    const bool active = t < C::ACTIVE;
+    const int r = t >> 2, h = t & 3;
+    const bool writer = active && h == 0;
+    const int flags = a.flags;
+    const bool sweep = (a.mode == MODE_SWEEP);
+    const bool need_d = sweep && (flags & F_NEED_D);
+    const bool touch_x = (flags & (F_UPD_X | F_SET_X | F_FINAL_X)) != 0;
+    double *vec = sVec + g * C::VECPAD;
+    double inv_scale = 1.0;
+    if (diag && ex.scale_div != nullptr) inv_scale = 1.0 / *ex.scale_div;
+
+    int seen = 0;  // last value read from `issued`
+    int64_t I = R0 + g;
+    int64_t p0 = 0, p1 = 0;
+    if (I < R1) {
+        p0 = diag ? I : a.row_ptr[I];
+        p1 = diag ? I + 1 : a.row_ptr[I + 1];
+    }
+    for (; I < R1; I += C::NG) {
+        // next row's extent (off the critical path)
+        const int64_t In = I + C::NG;
+        int64_t p0n = 0, p1n = 0;
+        if (In < R1) {
+            p0n = diag ? In : a.row_ptr[In];
+            p1n = diag ? In + 1 : a.row_ptr[In + 1];
+        }
+        const size_t gi = (size_t)I * B + r;
+        double rin_v = 0.0, dold = 0.0, xold = 0.0;
+        double dreg[C::SEGL];
+#pragma unroll
+        for (int c = 0; c < C::SEGL; ++c) dreg[c] = 0.0;
+        if (active) {
+            if (a.mode == MODE_RESID || sweep || (diag && ex.vout != nullptr)) rin_v = a.rin[gi];
+            if (sweep) dold = a.vin[gi];
+            if (touch_x && !(flags & F_SET_X)) xold = a.x[gi];
+            if (need_d) {
+                const double *dp = a.dinv + (size_t)I * BB + C::SEGL * t;
+#pragma unroll
+                for (int c = 0; c < C::SEGL; ++c) dreg[c] = __ldg(dp + c);
+            }
+        }
+        int n = (int)(p0 - P0);
+        int s = n % C::STAGES;
+        uint32_t ph = (uint32_t)(n / C::STAGES) & 1u;
+        double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0;
+        for (int64_t p = p0; p < p1; ++p, ++n) {
+            if (n >= seen) {
+                do {
+                    seen = *issued;
+                } while (n >= seen);
+            }
+            mbar_wait(&full[s], ph);
+            if (active) {
+                const double *A = sA + (size_t)s * BB + C::SEGL * t;
+                const double *xs = sX + s * B + C::SEGL * h;
+                acc0 = fma(A[0], xs[0], acc0);
+                acc1 = fma(A[1], xs[1], acc1);
+                acc2 = fma(A[2], xs[2], acc2);
+                acc0 = fma(A[3], xs[3], acc0);
+                acc1 = fma(A[4], xs[4], acc1);
+                acc2 = fma(A[5], xs[5], acc2);
+                acc0 = fma(A[6], xs[6], acc0);
+                acc1 = fma(A[7], xs[7], acc1);
+                acc2 = fma(A[8], xs[8], acc2);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[s]);
+            if (++s == C::STAGES) {
+                s = 0;
+                ph ^= 1u;
+            }
+        }
+        double acc = (acc0 + acc1) + acc2;
+        acc += __shfl_xor_sync(0xffffffffu, acc, 1);
+        acc += __shfl_xor_sync(0xffffffffu, acc, 2);
+
+        if (a.mode == MODE_SPMV) {
+            if (writer) a.out[gi] = acc;
+        } else if (a.mode == MODE_RESID) {
+            if (writer) a.out[gi] = rin_v - acc;
+        } else if (diag) {
+            const double dnew = a.c_z * (acc * inv_scale);
+            if (writer) {
+                a.dout[gi] = dnew;
+                if (ex.vout != nullptr) ex.vout[gi] = rin_v * inv_scale;
+                if (flags & F_FINAL_X) a.x[gi] = xold + dnew;
+            }
+        } else {
+            const double rnew = rin_v - acc;
+            if (writer) a.out[gi] = rnew;
+            if (!need_d) {
+                if (writer) {
+                    if (flags & F_SET_X) a.x[gi] = dold;
+                    else if (flags & F_UPD_X) a.x[gi] = xold + dold;
+                }
+            } else {
+                if (writer) vec[r] = rnew;
+                group_bar(g);
+                double z = 0.0;
+                if (active) {
+#pragma unroll
+                    for (int c = 0; c < C::SEGL; ++c) z = fma(dreg[c], vec[C::SEGL * h + c], z);
+                }
+                z += __shfl_xor_sync(0xffffffffu, z, 1);
+                z += __shfl_xor_sync(0xffffffffu, z, 2);
+                group_bar(g);
+                if (writer) {
+                    double dnew = a.c_z * z;
+                    if (a.c_d != 0.0) dnew = fma(a.c_d, dold, dnew);
+                    double xv;
+                    if (flags & F_SET_X) xv = dold;
+                    else {
+                        xv = xold;
+                        if (flags & F_UPD_X) xv += dold;
+                    }
+                    a.dout[gi] = dnew;
+                    if (flags & F_FINAL_X) xv += dnew;
+                    if (touch_x) a.x[gi] = xv;
+                }
+            }
+        }
+        p0 = p0n;
+        p1 = p1n;
+    }
+}
+
+}  // namespace mgk

@@ -108,13 +108,59 @@ __global__ void __launch_bounds__(256) dot_multi_kernel(const double *__restrict
     }
 }
 
+// ------------------------------------------------------------------------------------------------ GMRES state
+// Device-resident Arnoldi / Givens bookkeeping (one thread): nothing of a restart cycle needs the host.
+struct GmresDev {
+    double *H;     // (m+1) x m, column-major, leading dimension m+1 (upper triangular after rotations)
+    double *cs, *sn, *g, *y;
+    double *h1, *h2;   // the two classical Gram-Schmidt passes of the current column
+    double *nrm2;      // ||w||^2 after orthogonalisation / ||r||^2 at cycle begin / ||rhs||^2
+    double *hnext;     // h_{j+1,j} (or beta): divisor for the next basis vector
+    double *tol;       // absolute tolerance rtol*||rhs||
+    double *hist;      // hist[it] = residual estimate (absolute), it = 0..maxit
+    int *status;       // [0] done, [1] j_used, [2] it, [3] converged
+    int m, maxit;
+};
+
+// Column j: h = h1 + h2, h_{j+1,j} = ||w||, previous rotations, new rotation, residual estimate, stop test.
+// One thread.  Runs at the tail of the second Gram-Schmidt update (axpy_multi_kernel, last CTA).
+__device__ __forceinline__ void gmres_update_dev(const GmresDev &s, const int j) {
+    if (s.status[0] != 0) return;
+    double *col = s.H + (size_t)j * (s.m + 1);
+    for (int i = 0; i <= j; ++i) col[i] = s.h1[i] + s.h2[i];
+    const double hn = sqrt(fmax(*s.nrm2, 0.0));
+    col[j + 1] = hn;
+    *s.hnext = hn;
+    for (int i = 0; i < j; ++i) {
+        const double t = s.cs[i] * col[i] + s.sn[i] * col[i + 1];
+        col[i + 1] = -s.sn[i] * col[i] + s.cs[i] * col[i + 1];
+        col[i] = t;
+    }
+    const double denom = hypot(col[j], col[j + 1]);
+    s.cs[j] = col[j] / denom;
+    s.sn[j] = col[j + 1] / denom;
+    col[j] = denom;
+    col[j + 1] = 0.0;
+    s.g[j + 1] = -s.sn[j] * s.g[j];
+    s.g[j] = s.cs[j] * s.g[j];
+    const int it = s.status[2] + 1;
+    s.status[2] = it;
+    s.status[1] = j + 1;
+    const double est = fabs(s.g[j + 1]);
+    s.hist[it] = est;
+    const bool breakdown = (hn == 0.0);
+    if (est <= *s.tol || breakdown) { s.status[0] = 1; s.status[3] = 1; }
+    else if (it >= s.maxit) { s.status[0] = 1; }
+}
+
 // w += sign * sum_{i<k} coef[i] V_i ; optionally nrm2 = <w, w> of the result (same deterministic scheme).
 // If kdev != nullptr the live count is min(k, *kdev).
 __global__ void __launch_bounds__(256) axpy_multi_kernel(const double *__restrict__ V, const int64_t stride, const int k,
                                                          const int *__restrict__ kdev, const double *__restrict__ coef,
                                                          const double sign, double *__restrict__ w, const int64_t n,
                                                          double *__restrict__ partial, unsigned *__restrict__ counter,
-                                                         double *__restrict__ nrm2, const int *done) {
+                                                         double *__restrict__ nrm2, const int *done, const GmresDev upd,
+                                                         const int upd_j /* >= 0: Hessenberg/Givens update of column j */) {
     MG_EARLY_EXIT(done);
     __shared__ double cf[128];
     __shared__ double sh[8];
@@ -175,6 +221,7 @@ __global__ void __launch_bounds__(256) axpy_multi_kernel(const double *__restric
         if (threadIdx.x == 0) {
             *nrm2 = tot;
             *counter = 0;
+            if (upd_j >= 0) gmres_update_dev(upd, upd_j);
         }
     }
 }
@@ -203,20 +250,6 @@ __global__ void __launch_bounds__(256) hashed_start_kernel(double *__restrict__ 
     }
 }
 
-// ------------------------------------------------------------------------------------------------ GMRES state
-// Device-resident Arnoldi / Givens bookkeeping (one thread): nothing of a restart cycle needs the host.
-struct GmresDev {
-    double *H;     // (m+1) x m, column-major, leading dimension m+1 (upper triangular after rotations)
-    double *cs, *sn, *g, *y;
-    double *h1, *h2;   // the two classical Gram-Schmidt passes of the current column
-    double *nrm2;      // ||w||^2 after orthogonalisation / ||r||^2 at cycle begin / ||rhs||^2
-    double *hnext;     // h_{j+1,j} (or beta): divisor for the next basis vector
-    double *tol;       // absolute tolerance rtol*||rhs||
-    double *hist;      // hist[it] = residual estimate (absolute), it = 0..maxit
-    int *status;       // [0] done, [1] j_used, [2] it, [3] converged
-    int m, maxit;
-};
-
 __global__ void gmres_set_tol_kernel(GmresDev s, const double rtol) {
     *s.tol = rtol * sqrt(fmax(*s.nrm2, 0.0));
     s.status[0] = 0; s.status[1] = 0; s.status[2] = 0; s.status[3] = 0;
@@ -232,36 +265,6 @@ __global__ void gmres_begin_kernel(GmresDev s) {
     if (s.status[2] >= s.maxit) { s.status[0] = 1; return; }
     s.g[0] = beta;
     *s.hnext = beta;
-}
-
-// Column j: h = h1 + h2, h_{j+1,j} = ||w||, previous rotations, new rotation, residual estimate, stop test.
-__global__ void gmres_update_kernel(GmresDev s, const int j) {
-    if (s.status[0] != 0) return;
-    double *col = s.H + (size_t)j * (s.m + 1);
-    for (int i = 0; i <= j; ++i) col[i] = s.h1[i] + s.h2[i];
-    const double hn = sqrt(fmax(*s.nrm2, 0.0));
-    col[j + 1] = hn;
-    *s.hnext = hn;
-    for (int i = 0; i < j; ++i) {
-        const double t = s.cs[i] * col[i] + s.sn[i] * col[i + 1];
-        col[i + 1] = -s.sn[i] * col[i] + s.cs[i] * col[i + 1];
-        col[i] = t;
-    }
-    const double denom = hypot(col[j], col[j + 1]);
-    s.cs[j] = col[j] / denom;
-    s.sn[j] = col[j + 1] / denom;
-    col[j] = denom;
-    col[j + 1] = 0.0;
-    s.g[j + 1] = -s.sn[j] * s.g[j];
-    s.g[j] = s.cs[j] * s.g[j];
-    const int it = s.status[2] + 1;
-    s.status[2] = it;
-    s.status[1] = j + 1;
-    const double est = fabs(s.g[j + 1]);
-    s.hist[it] = est;
-    const bool breakdown = (hn == 0.0);
-    if (est <= *s.tol || breakdown) { s.status[0] = 1; s.status[3] = 1; }
-    else if (it >= s.maxit) { s.status[0] = 1; }
 }
 
 // Back substitution H y = g over the j_used columns of this cycle.

@@ -12,6 +12,7 @@
 #include <vector>
 
 #include "kernels_bsr.cuh"
+#include "kernels_bsr_tma.cuh"
 #include "kernels_setup.cuh"
 #include "kernels_vec.cuh"
 
@@ -30,6 +31,8 @@ struct Level {
     const double *vals = nullptr;
     int64_t *diag_pos = nullptr;
     double *dinv = nullptr;
+    int64_t *part = nullptr;  // TMA kernel: first block row of each persistent CTA (tma_grid + 1 entries)
+    int tma_grid = 0;
     double rho_est = 0.0, lam_min = 0.0, lam_max = 0.0;
     double *x = nullptr, *r = nullptr, *d[2] = {nullptr, nullptr}, *pe = nullptr, *rhs = nullptr;
     std::vector<int64_t> h_row_ptr;  // host copies of the pattern (Galerkin symbolic phase)
@@ -64,6 +67,8 @@ struct Gmres {
 struct mg_handle {
     mg_options opt{};
     int b = 0, n_pol = 0, n_phi = 0, n_levels = 0;
+    int sm_count = 148;
+    bool tma_ready = false;  // b == 36 and the kernel's shared-memory attribute is set
     cudaStream_t stream = nullptr;      // active stream: the caller's, or cap_stream while a graph is captured
     cudaStream_t cap_stream = nullptr;  // internal non-default stream (the legacy default stream cannot capture)
     std::vector<Level> lev;
@@ -210,7 +215,7 @@ inline int grid_for(int64_t n, int per_block, int cap = 148 * 16) {
 }
 
 // ------------------------------------------------------------------------------------------------ BSR launch
-int launch_bsr(mg_handle *h, const Level &L, BsrArgs a) {
+int launch_bsr(mg_handle *h, const Level &L, BsrArgs a, TmaExtra ex = TmaExtra{nullptr, nullptr, nullptr}) {
     a.row_ptr = L.row_ptr;
     a.col_idx = L.col_idx;
     a.vals = L.vals;
@@ -220,6 +225,18 @@ int launch_bsr(mg_handle *h, const Level &L, BsrArgs a) {
     const int kind = a.mode == MODE_SPMV ? MG_KIND_SPMV : a.mode == MODE_RESID ? MG_KIND_RESID : a.mode == MODE_PBJ ? MG_KIND_PBJ
                      : (a.flags & F_NEED_D) ? MG_KIND_SWEEP : MG_KIND_SWEEP_NOD;
     KindScope scope(h, L.index, kind);
+    if (h->tma_ready && h->opt.kernel_variant == 0 && L.part != nullptr) {
+        int grid = L.tma_grid;
+        ex.part = L.part;
+        if (a.mode == MODE_PBJ) {  // implicit block-diagonal stream: uniform split
+            ex.part = nullptr;
+            grid = (int)std::min<int64_t>(h->sm_count, L.n_brows);
+        }
+        LAUNCH(h, bsr_tma_kernel, grid, TmaCfg::THREADS, TmaCfg::SMEM, a, ex);
+        CU(cudaGetLastError());
+        return MG_OK;
+    }
+    if (ex.scale_div != nullptr || ex.vout != nullptr) return MG_EINVAL;  // fused scaling exists in the TMA kernel only
     switch (h->b) {
 #define BSR_CASE(B)                                                                                          \
     case B: {                                                                                                \
@@ -269,6 +286,18 @@ int pbj(mg_handle *h, const Level &L, const double *rin, double *dout, double c_
     a.flags = xacc ? F_FINAL_X : 0;
     a.done = done;
     return launch_bsr(h, L, a);
+}
+// vout = rin / *denom ; dout = Dinv vout   (TMA kernel only; vout may alias rin)
+int pbj_scaled(mg_handle *h, const Level &L, const double *rin, double *dout, const double *denom, double *vout,
+               const int *done) {
+    BsrArgs a{};
+    a.mode = MODE_PBJ;
+    a.rin = rin;
+    a.dout = dout;
+    a.c_z = 1.0;
+    a.done = done;
+    TmaExtra ex{nullptr, denom, vout};
+    return launch_bsr(h, L, a, ex);
 }
 int sweep(mg_handle *h, const Level &L, const double *vin, const double *rin, double *rout, double *x, double *dout,
           double c_d, double c_z, int flags) {
@@ -418,17 +447,19 @@ int gmres_start(mg_handle *h, Gmres &G, const double *rhs, double rtol) {
     return MG_OK;
 }
 // V[0] holds the residual r: beta = ||r||, stop test, g = beta e_1, V[0] /= beta.
-int gmres_cycle_begin(mg_handle *h, Gmres &G) {
+int gmres_cycle_begin(mg_handle *h, Gmres &G, bool normalize = true) {
     KindScope scope(h, G.level, MG_KIND_ORTH);
     const int *done = G.dev.status;
     LAUNCH(h, dot_multi_kernel, dim3(G.red_grid, 1), 256, 0, G.V, (int64_t)0, G.V, G.n, G.partial, G.counter, G.dev.nrm2,
            done);
     LAUNCH(h, gmres_begin_kernel, 1, 1, 0, G.dev);
-    MG(scale_div(h, G.V, G.V, G.n, G.dev.hnext, done));
+    if (normalize) MG(scale_div(h, G.V, G.V, G.n, G.dev.hnext, done));
     return MG_OK;
 }
-// V[j+1] holds w = A M v_j: two classical Gram-Schmidt passes against V[0..j], Hessenberg column, v_{j+1}.
-int gmres_orth(mg_handle *h, Gmres &G, int j) {
+// V[j+1] holds w = A M v_j: two classical Gram-Schmidt passes against V[0..j]; the tail of the second update
+// kernel does the Hessenberg column / Givens / stop test.  normalize: v_{j+1} = w / h_{j+1,j} here (otherwise the
+// caller folds the division into its next kernel).
+int gmres_orth(mg_handle *h, Gmres &G, int j, bool normalize = true) {
     KindScope scope(h, G.level, MG_KIND_ORTH);
     const int *done = G.dev.status;
     double *w = G.V + (size_t)(j + 1) * G.stride;
@@ -438,10 +469,9 @@ int gmres_orth(mg_handle *h, Gmres &G, int j) {
         LAUNCH(h, dot_multi_kernel, dim3(G.red_grid, j + 1), 256, 0, G.V, G.stride, w, G.n, G.partial, G.counter, hh,
                done);
         LAUNCH(h, axpy_multi_kernel, axpy_grid, 256, 0, G.V, G.stride, j + 1, (const int *)nullptr, hh, -1.0, w, G.n,
-               G.partial, G.counter + G.m + 1, pass == 1 ? G.dev.nrm2 : (double *)nullptr, done);
+               G.partial, G.counter + G.m + 1, pass == 1 ? G.dev.nrm2 : (double *)nullptr, done, G.dev, pass == 1 ? j : -1);
     }
-    LAUNCH(h, gmres_update_kernel, 1, 1, 0, G.dev, j);
-    MG(scale_div(h, w, w, G.n, G.dev.hnext, done));
+    if (normalize) MG(scale_div(h, w, w, G.n, G.dev.hnext, done));
     CU(cudaGetLastError());
     return MG_OK;
 }
@@ -451,7 +481,7 @@ int gmres_cycle_end(mg_handle *h, Gmres &G, double *out) {
     LAUNCH(h, gmres_solve_y_kernel, 1, 1, 0, G.dev);
     const int axpy_grid = (int)((G.n / 2 + 256) / 256);
     LAUNCH(h, axpy_multi_kernel, axpy_grid, 256, 0, G.flexible ? G.Z : G.V, G.stride, G.m, G.dev.status + 1, G.dev.y, 1.0,
-           out, G.n, G.partial, G.counter + G.m + 1, (double *)nullptr, (const int *)nullptr);
+           out, G.n, G.partial, G.counter + G.m + 1, (double *)nullptr, (const int *)nullptr, G.dev, -1);
     CU(cudaGetLastError());
     return MG_OK;
 }
@@ -467,12 +497,16 @@ int coarse_cycle_enqueue(mg_handle *h) {
     Level &L = h->lev.back();
     Gmres &G = h->coarse;
     const int *done = G.dev.status;
+    // TMA kernel: the division v_j = w / h_{j,j-1} rides in the PBJ apply that follows it (one launch, one pass)
+    const bool fused = h->tma_ready && h->opt.kernel_variant == 0 && L.part != nullptr;
     MG(residual(h, L, L.rhs, L.x, G.V, done));
-    MG(gmres_cycle_begin(h, G));
+    MG(gmres_cycle_begin(h, G, !fused));
     for (int j = 0; j < G.m; ++j) {
-        MG(pbj(h, L, G.V + (size_t)j * G.stride, L.d[0], 1.0, nullptr, done));
+        double *vj = G.V + (size_t)j * G.stride;
+        if (fused) MG(pbj_scaled(h, L, vj, L.d[0], G.dev.hnext, vj, done));  // v_j /= h ; d0 = D^-1 v_j
+        else MG(pbj(h, L, vj, L.d[0], 1.0, nullptr, done));
         MG(spmv(h, L, L.d[0], G.V + (size_t)(j + 1) * G.stride, done));
-        MG(gmres_orth(h, G, j));
+        MG(gmres_orth(h, G, j, !fused));
     }
     CU(cudaMemsetAsync(L.d[1], 0, (size_t)L.nvec * sizeof(double), h->stream));
     MG(gmres_cycle_end(h, G, L.d[1]));
@@ -640,6 +674,16 @@ void galerkin_symbolic(const Level &F, int n_pol, std::vector<int64_t> &crow_ptr
     }
 }
 
+// TMA kernel (b = 36): contiguous row ranges with equal block counts, one per persistent CTA.
+int setup_level_partition(mg_handle *h, Level &L) {
+    if (!h->tma_ready || L.n_brows == 0) return MG_OK;
+    L.tma_grid = (int)std::min<int64_t>(h->sm_count, L.n_brows);
+    MG(dalloc_t(h, &L.part, (size_t)L.tma_grid + 1));
+    LAUNCH(h, partition_rows_kernel, (L.tma_grid + 1 + 127) / 128, 128, 0, L.row_ptr, L.n_brows, L.nnzb, L.tma_grid, L.part);
+    CU(cudaGetLastError());
+    return MG_OK;
+}
+
 int alloc_level_vectors(mg_handle *h, Level &L) {
     const size_t n = (size_t)L.nvec + 2;
     MG(dalloc_t(h, &L.x, n));
@@ -743,6 +787,7 @@ int mg_options_default(mg_options *o) {
     o->maxit = 400;
     o->block_layout = 0;
     o->use_graphs = 1;
+    o->kernel_variant = 0;
     return MG_OK;
 }
 
@@ -752,6 +797,7 @@ static int validate_options(const mg_options &o) {
     if (o.coarse_mode < 0 || o.coarse_mode > 1 || !(o.coarse_rtol > 0.0)) return MG_EINVAL;
     if (o.coarse_restart < 1 || o.coarse_maxit < 1 || o.coarse_fixed_sweeps < 0) return MG_EINVAL;
     if (o.restart < 1 || o.maxit < 1 || o.block_layout != 0) return MG_EINVAL;
+    if (o.kernel_variant < 0 || o.kernel_variant > 1) return MG_EINVAL;
     return MG_OK;
 }
 
@@ -815,6 +861,16 @@ int mg_setup(mg_handle **out, const int64_t *row_ptr, const int32_t *col_idx, co
     if (cudaMemsetAsync(h->red_counter, 0, 8 * sizeof(unsigned), h->stream) != cudaSuccess)
         return fail(cuda_fail(cudaGetLastError(), "cudaMemsetAsync"));
 
+    {
+        int dev = 0, sms = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
+            h->sm_count = sms;
+        if (b == TmaCfg::B) {
+            if (cudaFuncSetAttribute(bsr_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TmaCfg::SMEM) != cudaSuccess)
+                return fail(cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute(bsr_tma_kernel)"));
+            h->tma_ready = true;
+        }
+    }
     Level &L0 = h->lev[0];
     L0.n_phi = n_phi;
     L0.n_brows = (int64_t)n_pol * n_phi;
@@ -833,6 +889,7 @@ int mg_setup(mg_handle **out, const int64_t *row_ptr, const int32_t *col_idx, co
     for (int l = 0; l < levels; ++l) {
         Level &L = h->lev[l];
         if ((rc = setup_level_pbj(h, L)) != MG_OK) return fail(rc);
+        if ((rc = setup_level_partition(h, L)) != MG_OK) return fail(rc);
         if ((rc = alloc_level_vectors(h, L)) != MG_OK) return fail(rc);
         if ((rc = power_rho(h, L, o.eig_iters, &L.rho_est)) != MG_OK) return fail(rc);
         set_bounds(h, L);
@@ -853,6 +910,11 @@ int mg_update_options(mg_handle *h, const mg_options *opt) {
     o.block_layout = h->opt.block_layout;
     if (validate_options(o) != MG_OK) return MG_EINVAL;
     const bool bounds = (o.cheb_lo != h->opt.cheb_lo) || (o.cheb_hi != h->opt.cheb_hi);
+    if (o.kernel_variant != h->opt.kernel_variant && h->coarse_graph) {  // the captured cycle holds the old kernels
+        cudaStreamSynchronize(h->stream);
+        cudaGraphExecDestroy(h->coarse_graph);
+        h->coarse_graph = nullptr;
+    }
     h->opt = o;
     if (bounds)
         for (auto &L : h->lev) set_bounds(h, L);

@@ -19,15 +19,22 @@ CASES = {
     "b5-generic-to-1-plane": dict(name="C0", mesh=(3, 8), n_phi=4, levels=3, b=5, seed=79),
     "b1": dict(name="C0", mesh=(3, 7), n_phi=6, levels=2, b=1, seed=80),
     "b36-nonaxi": dict(name="C3", mesh=(3, 10), n_phi=8, levels=3, seed=81),
+    # TMA-ring kernel: ~120 blocks per persistent CTA (the 20-stage ring wraps six times), ragged row ranges
+    "b36-ring-wraps": dict(name="C0", mesh=(8, 30), n_phi=8, levels=3, seed=82),
+    # fewer block rows than SMs on the coarsest level (CTAs with a single row, idle consumer groups)
+    "b36-few-rows": dict(name="C0", mesh=(3, 5), n_phi=8, levels=3, seed=83),
+    # the one-CTA-per-row 128-bit-load kernel at b = 36 (kernel_variant = 1)
+    "b36-ldg-variant": dict(name="C0", mesh=(4, 12), n_phi=8, levels=2, seed=84, opt=dict(kernel_variant=1)),
 }
 
 
 @pytest.fixture(scope="module", params=list(CASES))
 def case(request):
     kw = dict(CASES[request.param])
+    opt = kw.pop("opt", {})
     w = small(kw.pop("name"), **kw)
     H = oracle_hierarchy(w)
-    s = gpu_solver(w, inject_bounds_from=H)
+    s = gpu_solver(w, inject_bounds_from=H, **opt)
     yield w, H, s
     s.destroy()
 
@@ -110,9 +117,10 @@ def test_prolongation_of_plane_constant_field_is_exact(case):
         assert np.array_equal(to_np(xg), np.tile(plane, Lf.n_phi))
 
 
-def test_shuffled_numbering_spmv():
+@pytest.mark.parametrize("b", [12, 36])
+def test_shuffled_numbering_spmv(b):
     """configs[4] 'shuffled' variant: col_idx is arbitrary within a plane."""
-    w = small("C0", mesh=(6, 20), n_phi=4, levels=1, b=12, seed=90, shuffle=True)
+    w = small("C0", mesh=(6, 20), n_phi=4, levels=1, b=b, seed=90, shuffle=True)
     H = oracle_hierarchy(w)
     s = gpu_solver(w, inject_bounds_from=H)
     try:
