@@ -200,7 +200,7 @@ def reference_arm(args):
     opt = dict(nu_pre=2, nu_post=2, restart=100, coarse_restart=50)
     counts = REFERENCE_COUNTS.get(args.workload, REFERENCE_COUNTS["C1"])
     total_bytes = solve_bytes_from_counts(sizes, counts["outer_iters"], counts["coarse_iters"], opt)
-    per_step = max(2.0, min(15.0, 150.0 / max(1, args.steps + args.warmup)))
+    per_step = max(0.05, min(args.cpu_seconds, 150.0 / max(1, args.steps + args.warmup)))
     for _ in range(args.warmup):
         oracle_sample(w, per_step)
     vals, desc, threads = [], "", 1

@@ -177,7 +177,10 @@ __global__ void __launch_bounds__(TmaCfg::THREADS, 1) bsr_tma_kernel(const BsrAr
                 if (lane == 0) {
                     mbar_wait(&empty[s], ph ^ 1u);
                     mbar_expect_tx(&full[s], (uint32_t)((BB + B) * sizeof(double)));
-                    bulk_g2s_hint(sA + (size_t)s * BB, stream + (size_t)(P0 + base + i) * BB, BB * sizeof(double), &full[s], pol);
+                    // the matrix stream is read once per launch: evict-first keeps the vectors, the Krylov basis and (on
+                    // small levels) Dinv resident in the 126 MB L2; Dinv itself (PBJ apply) is loaded with the default policy
+                    if (diag) bulk_g2s(sA + (size_t)s * BB, stream + (size_t)(P0 + base + i) * BB, BB * sizeof(double), &full[s]);
+                    else bulk_g2s_hint(sA + (size_t)s * BB, stream + (size_t)(P0 + base + i) * BB, BB * sizeof(double), &full[s], pol);
                     bulk_g2s(sX + s * B, xsrc + (size_t)j * B, B * sizeof(double), &full[s]);
                     __threadfence_block();
                     *issued = base + i + 1;
