@@ -111,6 +111,20 @@ class ClockSampler:
         return out
 
 
+def measured_traffic(workload: str, level: int, kind: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
+    (profiles/r01_dram_traffic.csv; commands in profiles/r01_tma_kernel.md), or None."""
+    import csv
+    path = os.path.join(ROOT, "profiles", "r01_dram_traffic.csv")
+    if not os.path.exists(path):
+        return None
+    with open(path) as f:
+        for row in csv.DictReader(f):
+            if row["workload"] == workload and int(row["level"]) == level and row["kind"] == kind:
+                return int(row["dram_bytes_per_launch"])
+    return None
+
+
 def level_sizes(solver):
     from paper_2506_16676_b200.traffic import LevelSize
     out = []
@@ -322,7 +336,8 @@ def cuda_arm(args):
         top = next((d for d in detail if d["bytes_per_launch"]), None)
         if top:
             roof = {"bound": "hbm", "kernel": f"bsr kernel, kind {top['kind']}, level {top['level']}", "achieved": top["GBps"],
-                    "peak": peak, "unit": "GB/s", "frac": top["frac"], "traffic": None, "peak_source": peak_src,
+                    "peak": peak, "unit": "GB/s", "frac": top["frac"],
+                    "traffic": measured_traffic(w.name, top["level"], top["kind"]), "peak_source": peak_src,
                     "bytes_per_launch": top["bytes_per_launch"], "mean_us": top["mean_us"],
                     "share_of_step": top["share_of_step"], "frac_of_8TBs_nominal": top["GBps"] / 8000.0}
         # ---- oracle timed beside it (rank 0, N = 1 only)
