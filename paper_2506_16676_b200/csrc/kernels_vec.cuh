@@ -3,6 +3,7 @@
 // (batched dots with warp-shuffle reductions, batched axpys) and the device-resident Givens/Hessenberg
 // bookkeeping that lets a whole GMRES restart cycle run without a host round trip.
 #pragma once
+#include <cooperative_groups.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -224,6 +225,210 @@ __global__ void __launch_bounds__(256) axpy_multi_kernel(const double *__restric
             if (upd_j >= 0) gmres_update_dev(upd, upd_j);
         }
     }
+}
+
+// ------------------------------------------------------------------------------------------------ fused CGS2
+// One cooperative launch per Arnoldi step instead of four kernels: both classical Gram-Schmidt passes, the norm of
+// the result and the Hessenberg/Givens update.  CTA c owns the slice [c*slice, (c+1)*slice) of the vectors: it
+// keeps its slice of w in shared memory for the whole step and caches the slices of the first `cap` basis vectors
+// there while it reads them for the first dots, so that the first update, the second dots and the second update
+// run out of shared memory (the remaining vectors are re-read through L2).  The two global reductions (h1, h2)
+// are grid-wide barriers; every CTA then sums the per-CTA partials itself, in a fixed order (deterministic).
+struct OrthArgs {
+    const double *V;
+    int64_t stride;
+    int j;                 // orthogonalise against V_0..V_j
+    double *w;             // V_{j+1}, updated in place
+    int64_t n;
+    double *partial;       // [gridDim.x][ld]
+    double *nrm_partial;   // [gridDim.x]
+    unsigned *counter;     // ticket of the final norm, zero-initialised, self-resetting
+    GmresDev dev;
+    const int *done;
+    int slice;             // elements per CTA, even
+    int cap;               // basis vectors cached in shared memory
+    int ld;                // >= m + 1
+};
+#ifndef MG_ORTH_STAMP   // development probe: per-phase clock stamps (compiled out in the library)
+#define MG_ORTH_STAMP(k)
+#endif
+constexpr int ORTH_THREADS = 512;
+constexpr int ORTH_MAX_GRID = 152;          // 8 * 19: the cross-CTA reduction unrolls over 19 loads per thread
+constexpr int ORTH_SCRATCH = 8 * 64 + 32;   // doubles of reduction scratch (+ 2*ld for the half-slice dots)
+inline size_t orth_smem_bytes(int slice, int ld, int cap) {
+    return sizeof(double) * ((size_t)slice + 3 * (size_t)ld + ORTH_SCRATCH + (size_t)cap * slice);
+}
+
+// <src_slice, ws> over the double2 range [start, end), 8 independent 128-bit loads in flight per lane;
+// optionally copies the source into the shared-memory cache on the way.
+__device__ __forceinline__ double orth_dot_range(const double2 *__restrict__ src2, const double2 *__restrict__ ws2,
+                                                 double2 *cache2, const int start, const int end, const int lane) {
+    double acc0 = 0.0, acc1 = 0.0;
+    for (int k0 = start + lane; k0 < end; k0 += 32 * 8) {
+        double2 v[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const int e = k0 + 32 * u;
+            v[u] = (e < end) ? src2[e] : make_double2(0.0, 0.0);
+        }
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const int e = k0 + 32 * u;
+            if (e < end) {
+                if (cache2 != nullptr) cache2[e] = v[u];
+                const double2 wv = ws2[e];
+                acc0 = fma(v[u].x, wv.x, acc0);
+                acc1 = fma(v[u].y, wv.y, acc1);
+            }
+        }
+    }
+    return acc0 + acc1;
+}
+
+__global__ void __launch_bounds__(ORTH_THREADS, 1) gmres_orth_fused_kernel(const OrthArgs a) {
+    namespace cg = cooperative_groups;
+    cg::grid_group grid = cg::this_grid();
+    if (a.done != nullptr && *a.done != 0) return;   // written by an earlier kernel: every CTA takes the same branch
+    extern __shared__ __align__(16) double orth_sm[];
+    double *ws = orth_sm;                 // [slice]   this CTA's slice of w
+    double *hs = ws + a.slice;            // [ld]      coefficients of the current pass
+    double *hd = hs + a.ld;               // [2 * ld]  half-slice dot products
+    double *red = hd + 2 * a.ld;          // [ORTH_SCRATCH]
+    double *vc = red + ORTH_SCRATCH;      // [cap][slice] cached slices of V_0..V_{cap-1}
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int NW = ORTH_THREADS / 32;
+    const int G = gridDim.x;
+    const int64_t e0 = (int64_t)blockIdx.x * a.slice;
+    int len = 0;
+    if (e0 < a.n) len = (int)((a.n - e0 < (int64_t)a.slice) ? (a.n - e0) : (int64_t)a.slice);
+    const int len2 = len >> 1;            // 128-bit part; an odd last element (odd n only) is handled by one lane
+    const int half2 = (len2 + 1) >> 1;
+    const bool odd = (len & 1) != 0;
+    const int slice2 = a.slice >> 1;
+    const double2 *ws2 = reinterpret_cast<const double2 *>(ws);
+    MG_ORTH_STAMP(0);
+    for (int e = tid; e < len; e += ORTH_THREADS) ws[e] = a.w[e0 + e];
+    __syncthreads();
+    MG_ORTH_STAMP(1);
+    const int nvec = a.j + 1;
+    const int nc = nvec < a.cap ? nvec : a.cap;
+    for (int pass = 0; pass < 2; ++pass) {
+        // ---- dots of the slice with V_0..V_j: work item = (vector, half of the slice), one warp per item
+        for (int item = warp; item < 2 * nvec; item += NW) {
+            const int i = item >> 1, hf = item & 1;
+            const bool cached = i < a.cap;
+            const int start = hf * half2, end = (hf == 0) ? (half2 < len2 ? half2 : len2) : len2;
+            const double *vg = a.V + (size_t)i * a.stride + e0;
+            double *vs = vc + (size_t)(cached ? i : 0) * a.slice;
+            const bool from_smem = (pass == 1 && cached);
+            double s = orth_dot_range(reinterpret_cast<const double2 *>(from_smem ? vs : vg), ws2,
+                                      (pass == 0 && cached) ? reinterpret_cast<double2 *>(vs) : nullptr, start, end, lane);
+            if (odd && hf == 1 && lane == 0) {
+                const double v = from_smem ? vs[len - 1] : vg[len - 1];
+                if (pass == 0 && cached) vs[len - 1] = v;
+                s = fma(v, ws[len - 1], s);
+            }
+            s = warp_sum(s);
+            if (lane == 0) hd[item] = s;
+        }
+        __syncthreads();
+        for (int i = tid; i < nvec; i += ORTH_THREADS) a.partial[(size_t)blockIdx.x * a.ld + i] = hd[2 * i] + hd[2 * i + 1];
+        MG_ORTH_STAMP(2 + 4 * pass);
+        grid.sync();
+        MG_ORTH_STAMP(3 + 4 * pass);
+        // ---- h_i = sum over CTAs: 8 interleaved sub-ranges in parallel (19 independent loads each), fixed order
+        double *hout = (pass == 0) ? a.dev.h1 : a.dev.h2;
+        for (int i0 = 0; i0 < nvec; i0 += 64) {
+            const int il = tid & 63, q = tid >> 6, i = i0 + il;
+            double pv[ORTH_MAX_GRID / 8];
+#pragma unroll
+            for (int u = 0; u < ORTH_MAX_GRID / 8; ++u) {
+                const int c = q + 8 * u;
+                pv[u] = (i < nvec && c < G) ? __ldcg(a.partial + (size_t)c * a.ld + i) : 0.0;
+            }
+            double s = 0.0;
+#pragma unroll
+            for (int u = 0; u < ORTH_MAX_GRID / 8; ++u) s += pv[u];
+            red[q * 64 + il] = s;
+            __syncthreads();
+            if (q == 0 && i < nvec) {
+                double t = 0.0;
+#pragma unroll
+                for (int qq = 0; qq < 8; ++qq) t += red[qq * 64 + il];
+                hs[i] = t;
+                if (blockIdx.x == 0) hout[i] = t;
+            }
+            __syncthreads();
+        }
+        MG_ORTH_STAMP(4 + 4 * pass);
+        // ---- w_slice -= sum_i h_i V_i : one double2 per thread, two independent accumulator pairs
+        for (int e = tid; e < len2; e += ORTH_THREADS) {
+            double2 s0 = make_double2(0.0, 0.0), s1 = make_double2(0.0, 0.0);
+            const double2 *c2 = reinterpret_cast<const double2 *>(vc) + e;
+            int i = 0;
+#pragma unroll 4
+            for (; i + 1 < nc; i += 2) {
+                const double2 v0 = c2[(size_t)i * slice2], v1 = c2[(size_t)(i + 1) * slice2];
+                const double h0 = hs[i], h1 = hs[i + 1];
+                s0.x = fma(h0, v0.x, s0.x); s0.y = fma(h0, v0.y, s0.y);
+                s1.x = fma(h1, v1.x, s1.x); s1.y = fma(h1, v1.y, s1.y);
+            }
+            if (i < nc) {
+                const double2 v0 = c2[(size_t)i * slice2];
+                s0.x = fma(hs[i], v0.x, s0.x); s0.y = fma(hs[i], v0.y, s0.y);
+            }
+            const double2 *g2 = reinterpret_cast<const double2 *>(a.V + e0) + e;
+            const size_t st2 = (size_t)(a.stride >> 1);
+#pragma unroll 8
+            for (i = nc; i < nvec; ++i) {
+                const double2 v0 = __ldg(g2 + (size_t)i * st2);
+                s1.x = fma(hs[i], v0.x, s1.x); s1.y = fma(hs[i], v0.y, s1.y);
+            }
+            double2 wv = reinterpret_cast<double2 *>(ws)[e];
+            wv.x -= s0.x + s1.x;
+            wv.y -= s0.y + s1.y;
+            reinterpret_cast<double2 *>(ws)[e] = wv;
+        }
+        if (odd && tid == 0) {
+            double acc = 0.0;
+            for (int i = 0; i < nvec; ++i)
+                acc = fma(hs[i], (i < a.cap) ? vc[(size_t)i * a.slice + len - 1] : a.V[(size_t)i * a.stride + e0 + len - 1], acc);
+            ws[len - 1] -= acc;
+        }
+        __syncthreads();
+        MG_ORTH_STAMP(5 + 4 * pass);
+    }
+    // ---- write back, ||w||^2, Hessenberg column / Givens / stop test in the last CTA
+    double sq = 0.0;
+    for (int e = tid; e < len; e += ORTH_THREADS) {
+        const double v = ws[e];
+        a.w[e0 + e] = v;
+        sq = fma(v, v, sq);
+    }
+    sq = warp_sum(sq);
+    if (lane == 0) red[warp] = sq;
+    __syncthreads();
+    __shared__ bool last;
+    if (tid == 0) {
+        double t = 0.0;
+        for (int k = 0; k < NW; ++k) t += red[k];
+        a.nrm_partial[blockIdx.x] = t;
+        __threadfence();
+        last = (atomicAdd(a.counter, 1u) == (unsigned)(G - 1));
+    }
+    __syncthreads();
+    if (last && warp == 0) {
+        __threadfence();
+        double t = 0.0;
+        for (int c = lane; c < G; c += 32) t += __ldcg(a.nrm_partial + c);
+        t = warp_sum(t);
+        if (lane == 0) {
+            *a.dev.nrm2 = t;
+            *a.counter = 0;
+            gmres_update_dev(a.dev, a.j);
+        }
+    }
+    MG_ORTH_STAMP(10);
 }
 
 // dst = src / *denom   (v_{j+1} = w / h_{j+1,j}); dst may equal src.

@@ -60,6 +60,12 @@ struct Gmres {
     bool flexible = false;
     bool ready = false;
     int level = 0;  // level whose vectors this engine orthogonalises (profiling only)
+    // fused cooperative CGS2 step (gmres_orth_fused_kernel)
+    bool fused_ok = false;
+    int orth_grid = 0, orth_slice = 0, orth_cap = 0, orth_ld = 0;
+    size_t orth_smem = 0;
+    double *orth_partial = nullptr, *orth_nrm = nullptr;
+    unsigned *orth_counter = nullptr;
 };
 
 }  // namespace
@@ -68,6 +74,7 @@ struct mg_handle {
     mg_options opt{};
     int b = 0, n_pol = 0, n_phi = 0, n_levels = 0;
     int sm_count = 148;
+    bool coop_ok = false;    // cooperative launches available and gmres_orth_fused_kernel's shared memory opted in
     bool tma_ready = false;  // b == 36 and the kernel's shared-memory attribute is set
     cudaStream_t stream = nullptr;      // active stream: the caller's, or cap_stream while a graph is captured
     cudaStream_t cap_stream = nullptr;  // internal non-default stream (the legacy default stream cannot capture)
@@ -433,6 +440,25 @@ int gmres_alloc(mg_handle *h, Gmres &G, int64_t n, int m, int maxit, bool flexib
     MG(dalloc_t(h, &d.hist, (size_t)maxit + 2));
     MG(dalloc_t(h, &d.status, 4));
     CU(cudaMemsetAsync(d.status, 0, 4 * sizeof(int), h->stream));
+    // fused CGS2 step: one persistent CTA per SM, the slice of w (and as many basis slices as fit) in shared memory
+    G.fused_ok = false;
+    if (h->coop_ok && n > 0) {
+        const size_t budget = 220 * 1024;
+        G.orth_grid = (int)std::min<int64_t>(std::min(h->sm_count, ORTH_MAX_GRID), (n + 1) / 2);
+        G.orth_slice = (int)(((n + G.orth_grid - 1) / G.orth_grid + 1) / 2 * 2);
+        G.orth_grid = (int)((n + G.orth_slice - 1) / G.orth_slice);
+        G.orth_ld = (m + 2) / 2 * 2;
+        if (orth_smem_bytes(G.orth_slice, G.orth_ld, 0) <= budget) {
+            const size_t left = budget - orth_smem_bytes(G.orth_slice, G.orth_ld, 0);
+            G.orth_cap = (int)std::min<size_t>(left / (sizeof(double) * G.orth_slice), (size_t)m + 1);
+            G.orth_smem = orth_smem_bytes(G.orth_slice, G.orth_ld, G.orth_cap);
+            MG(dalloc_t(h, &G.orth_partial, (size_t)G.orth_grid * G.orth_ld));
+            MG(dalloc_t(h, &G.orth_nrm, (size_t)G.orth_grid));
+            MG(dalloc_t(h, &G.orth_counter, 2));
+            CU(cudaMemsetAsync(G.orth_counter, 0, 2 * sizeof(unsigned), h->stream));
+            G.fused_ok = true;
+        }
+    }
     G.ready = true;
     return MG_OK;
 }
@@ -463,6 +489,31 @@ int gmres_orth(mg_handle *h, Gmres &G, int j, bool normalize = true) {
     KindScope scope(h, G.level, MG_KIND_ORTH);
     const int *done = G.dev.status;
     double *w = G.V + (size_t)(j + 1) * G.stride;
+    if (G.fused_ok && h->opt.kernel_variant == 0) {
+        OrthArgs oa{};
+        oa.V = G.V;
+        oa.stride = G.stride;
+        oa.j = j;
+        oa.w = w;
+        oa.n = G.n;
+        oa.partial = G.orth_partial;
+        oa.nrm_partial = G.orth_nrm;
+        oa.counter = G.orth_counter;
+        oa.dev = G.dev;
+        oa.done = done;
+        oa.slice = G.orth_slice;
+        oa.cap = G.orth_cap;
+        oa.ld = G.orth_ld;
+        void *params[] = {&oa};
+        ProfPair pp;
+        const bool prof = prof_begin(h, pp);
+        CU(cudaLaunchCooperativeKernel((const void *)gmres_orth_fused_kernel, dim3(G.orth_grid), dim3(ORTH_THREADS), params,
+                                       G.orth_smem, h->stream));
+        if (prof) prof_end(h, pp);
+        count_launch(h);
+        if (normalize) MG(scale_div(h, w, w, G.n, G.dev.hnext, done));
+        return MG_OK;
+    }
     const int axpy_grid = (int)((G.n / 2 + 256) / 256);
     for (int pass = 0; pass < 2; ++pass) {
         double *hh = pass == 0 ? G.dev.h1 : G.dev.h2;
@@ -534,7 +585,7 @@ int coarse_solve_internal(mg_handle *h) {
     CU(cudaMemsetAsync(L.x, 0, (size_t)L.nvec * sizeof(double), h->stream));
     MG(gmres_start(h, G, L.rhs, h->opt.coarse_rtol));
     const bool use_graph = h->opt.use_graphs && !h->profiling;
-    if (use_graph && !h->coarse_graph) {
+    for (int attempt = 0; use_graph && !h->coarse_graph && attempt < 2; ++attempt) {
         cudaGraph_t graph = nullptr;
         if (!h->cap_stream) CU(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
         cudaStream_t user_stream = h->stream;
@@ -547,15 +598,20 @@ int coarse_solve_internal(mg_handle *h) {
         h->capturing = false;
         h->stream = user_stream;
         cudaError_t e = cudaStreamEndCapture(h->cap_stream, &graph);
-        if (rc != MG_OK) {
-            if (graph) cudaGraphDestroy(graph);
-            return rc;
+        if (e == cudaSuccess && rc == MG_OK) {
+            h->coarse_graph_kernels = h->capture_count;
+            e = cudaGraphInstantiate(&h->coarse_graph, graph, 0);
         }
-        if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture");
-        h->coarse_graph_kernels = h->capture_count;
-        e = cudaGraphInstantiate(&h->coarse_graph, graph, 0);
-        cudaGraphDestroy(graph);
-        if (e != cudaSuccess) return cuda_fail(e, "cudaGraphInstantiate");
+        if (graph) cudaGraphDestroy(graph);
+        if (e == cudaSuccess && rc == MG_OK) break;
+        cudaGetLastError();
+        h->coarse_graph = nullptr;
+        if (attempt == 0 && G.fused_ok) {  // a cooperative node the graph cannot hold: capture the four-kernel CGS2 instead
+            G.fused_ok = false;
+            continue;
+        }
+        if (rc != MG_OK) return rc;
+        return cuda_fail(e, "capture of the coarse GMRES cycle");
     }
     int st[4] = {0, 0, 0, 0};
     do {
@@ -865,6 +921,12 @@ int mg_setup(mg_handle **out, const int64_t *row_ptr, const int32_t *col_idx, co
         int dev = 0, sms = 0;
         if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
             h->sm_count = sms;
+        int coop = 0;
+        if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) == cudaSuccess && coop &&
+            cudaFuncSetAttribute(gmres_orth_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024) == cudaSuccess)
+            h->coop_ok = true;
+        else
+            cudaGetLastError();
         if (b == TmaCfg::B) {
             if (cudaFuncSetAttribute(bsr_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TmaCfg::SMEM) != cudaSuccess)
                 return fail(cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute(bsr_tma_kernel)"));
