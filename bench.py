@@ -171,10 +171,11 @@ def oracle_sample(w, seconds: float = 15.0):
 
 
 def orth_bytes(iters, restart, vec_bytes):
-    """CGS2 traffic of ``iters`` Arnoldi steps of GMRES(restart): step j reads V_0..V_j four times (+ w)."""
+    """Algorithmic CGS2 traffic of ``iters`` Arnoldi steps of GMRES(restart): step j must read V_0..V_j once (the fused
+    kernel keeps the slices on chip for the second pass) plus a few passes over w."""
     full, rem = divmod(int(iters), int(restart))
-    cyc = sum(4 * (j + 1) + 8 for j in range(restart))
-    return (full * cyc + sum(4 * (j + 1) + 8 for j in range(rem))) * vec_bytes
+    cyc = sum((j + 1) + 8 for j in range(restart))
+    return (full * cyc + sum((j + 1) + 8 for j in range(rem))) * vec_bytes
 
 
 def solve_bytes_from_counts(sizes, outer_iters, coarse_iters, opt):
@@ -315,7 +316,7 @@ def cuda_arm(args):
 
     # ---- roofline: a short event-bracketed pass (same inputs, a few outer iterations) gives mean kernel durations
     peak, peak_src = measured_peaks()
-    roof, detail, cpu = None, [], None
+    roof, detail, cpu, vcycle_roof = None, [], None, None
     if rank == 0:
         s.update_options(maxit=min(opt["maxit"], 2))
         s.profile_reset()
@@ -348,6 +349,32 @@ def cuda_arm(args):
                     "traffic": measured_traffic(w.name, top["level"], top["kind"]), "peak_source": peak_src,
                     "bytes_per_launch": top["bytes_per_launch"], "mean_us": top["mean_us"],
                     "share_of_step": top["share_of_step"], "frac_of_8TBs_nominal": top["GBps"] / 8000.0}
+        # ---- V-cycle roofline, reported twice: (i) one mg_vcycle in the pinned coarse mode (coarsest level = 8
+        # Chebyshev-PBJ sweeps: every byte is a smoother/transfer byte), CUDA events around 5 calls; (ii) the complete
+        # outer iteration of the timed solve (V-cycle with its measured coarse GMRES steps + SpMV + CGS2).
+        from paper_2506_16676_b200.traffic import vcycle_bytes
+        s.update_options(coarse_mode=1)
+        rv = torch.from_numpy(w.rhs).to(dev)
+        zv = s.new()
+        for _ in range(2):
+            s.vcycle(rv, zv)
+        v0, v1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        v0.record()
+        for _ in range(5):
+            s.vcycle(rv, zv)
+        v1.record()
+        torch.cuda.synchronize()
+        s.update_options(coarse_mode=opt["coarse_mode"])
+        vc_ms = v0.elapsed_time(v1) / 5
+        vc_bytes = vcycle_bytes(sizes, opt["nu_pre"], opt["nu_post"], coarse_sweeps=s.opt.coarse_fixed_sweeps)
+        solve_bytes = solve_bytes_from_counts(sizes, info["iters"], info["coarse_iters_total"], opt)
+        vcycle_roof = {
+            "pinned_coarse_mode": {"ms": vc_ms, "bytes": vc_bytes, "GBps": vc_bytes / vc_ms / 1e6,
+                                   "frac_of_measured_peak": vc_bytes / vc_ms / 1e6 / peak, "frac_of_8TBs_nominal": vc_bytes / vc_ms / 1e6 / 8000.0},
+            "complete_outer_iteration": {"ms": 1e3 * t_dev / max(1, info["iters"]), "bytes": solve_bytes / max(1, info["iters"]),
+                                         "GBps": solve_bytes / t_dev / 1e9, "frac_of_measured_peak": solve_bytes / t_dev / 1e9 / peak,
+                                         "frac_of_8TBs_nominal": solve_bytes / t_dev / 1e9 / 8000.0,
+                                         "coarse_steps_per_cycle": info["coarse_iters_total"] / max(1, info["iters"])}}
         # ---- oracle timed beside it (rank 0, N = 1 only)
         if world == 1 and not args.no_cpu_baseline:
             gbs, dt, threads, desc = oracle_sample(w, args.cpu_seconds)
@@ -377,7 +404,7 @@ def cuda_arm(args):
                            "outer_iters": info["iters"], "coarse_iters": info["coarse_iters_total"], "rel_res": info["rel_res"],
                            "max_abs_x": x_dev_check},
                 "e2e": {"value": t_e2e, "unit": UNIT, "h2d_bytes_per_step": 8 * n, "d2h_bytes_per_step": 8 * n},
-                "gpu_launches": launches, "clocks": clocks, "roofline": roof, "cpu_baseline": cpu,
+                "gpu_launches": launches, "clocks": clocks, "roofline": roof, "vcycle_roofline": vcycle_roof, "cpu_baseline": cpu,
                 "throughput": {"value": world / t_dev, "unit": "solves/s"}, "truncated": args.max_outer > 0,
                 "kernels": detail[:12]}
         print(json.dumps(line), flush=True)

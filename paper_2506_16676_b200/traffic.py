@@ -56,8 +56,9 @@ class LevelSize:
 
     def gmres_iteration(self, j: int) -> int:
         """One right-PBJ-preconditioned GMRES step with j previous basis vectors, CGS2: A, D^-1 once; the basis
-        V_0..V_j read four times (two dot passes, two update passes); w read/written a few times."""
-        return self.matrix_bytes + self.dinv_bytes + (4 * (j + 1) + 8) * self.vec_bytes
+        V_0..V_j read once (what the method must move: the second Gram-Schmidt pass can run from on-chip copies);
+        w and the work vectors read/written a few times."""
+        return self.matrix_bytes + self.dinv_bytes + ((j + 1) + 8) * self.vec_bytes
 
     def by_kind(self, kind: str) -> int:
         return getattr(self, kind)()
