@@ -47,8 +47,8 @@ struct TmaCfg {
 // extra arguments of the TMA kernel (the common ones are BsrArgs)
 struct TmaExtra {
     const int64_t *part;      // [gridDim.x + 1] first block row of every CTA (nullptr: uniform split, implicit diagonal)
-    const double *scale_div;  // PBJ mode, optional: the input is rin / *scale_div
-    double *vout;             // PBJ mode, optional: vout_I = rin_I / *scale_div
+    const double *scale_div;  // PBJ and SPMV modes, optional: the input vector is (rin | vin) / *scale_div
+    double *vout;             // PBJ and SPMV modes, optional: vout_I = (rin_I | vin_I) / *scale_div (PBJ: may alias rin)
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -205,7 +205,8 @@ __global__ void __launch_bounds__(TmaCfg::THREADS, 1) bsr_tma_kernel(const BsrAr
     const bool touch_x = (flags & (F_UPD_X | F_SET_X | F_FINAL_X)) != 0;
     double *vec = sVec + g * C::VECPAD;
     double inv_scale = 1.0;
-    if (diag && ex.scale_div != nullptr) inv_scale = 1.0 / *ex.scale_div;
+    const bool spmv_scaled = (a.mode == MODE_SPMV) && ex.scale_div != nullptr;
+    if ((diag || spmv_scaled) && ex.scale_div != nullptr) inv_scale = 1.0 / *ex.scale_div;
 
     int seen = 0;  // last value read from `issued`
     int64_t I = R0 + g;
@@ -229,7 +230,7 @@ __global__ void __launch_bounds__(TmaCfg::THREADS, 1) bsr_tma_kernel(const BsrAr
         for (int c = 0; c < C::SEGL; ++c) dreg[c] = 0.0;
         if (active) {
             if (a.mode == MODE_RESID || sweep || (diag && ex.vout != nullptr)) rin_v = a.rin[gi];
-            if (sweep) dold = a.vin[gi];
+            if (sweep || (spmv_scaled && ex.vout != nullptr)) dold = a.vin[gi];
             if (touch_x && !(flags & F_SET_X)) xold = a.x[gi];
             if (need_d) {
                 const double *dp = a.dinv + (size_t)I * BB + C::SEGL * t;
@@ -273,7 +274,10 @@ __global__ void __launch_bounds__(TmaCfg::THREADS, 1) bsr_tma_kernel(const BsrAr
         acc += __shfl_xor_sync(0xffffffffu, acc, 2);
 
         if (a.mode == MODE_SPMV) {
-            if (writer) a.out[gi] = acc;
+            if (writer) {
+                a.out[gi] = spmv_scaled ? acc * inv_scale : acc;
+                if (spmv_scaled && ex.vout != nullptr) ex.vout[gi] = dold * inv_scale;   // the normalised input vector
+            }
         } else if (a.mode == MODE_RESID) {
             if (writer) a.out[gi] = rin_v - acc;
         } else if (diag) {

@@ -166,4 +166,31 @@ __global__ void __launch_bounds__(128) galerkin_numeric_kernel(const int64_t *__
     }
 }
 
+// Ahat_p = A_p * Dinv_{col(p)}: the right-PBJ-preconditioned operator A D^-1 of the coarsest-level GMRES as ONE
+// block-CSR matrix with A's pattern ("right-preconditioned ... M_c = D^-1").  A GMRES
+// step is then a single SpMV instead of a PBJ apply followed by an SpMV.  One CTA per block; plain triple loop in
+// FP64 (k innermost in stored order), b <= 64.
+__global__ void __launch_bounds__(256) right_scale_blocks_kernel(const int32_t *__restrict__ col_idx,
+                                                                 const double *__restrict__ vals,
+                                                                 const double *__restrict__ dinv, double *__restrict__ out,
+                                                                 const int b) {
+    extern __shared__ double rs_sm[];
+    const int bb = b * b;
+    double *As = rs_sm, *Ds = rs_sm + bb;
+    const int64_t p = blockIdx.x;
+    const double *Ap = vals + (size_t)p * bb;
+    const double *Dp = dinv + (size_t)col_idx[p] * bb;
+    for (int e = threadIdx.x; e < bb; e += blockDim.x) {
+        As[e] = Ap[e];
+        Ds[e] = Dp[e];
+    }
+    __syncthreads();
+    for (int e = threadIdx.x; e < bb; e += blockDim.x) {
+        const int r = e / b, c = e - r * b;
+        double acc = 0.0;
+        for (int k = 0; k < b; ++k) acc = fma(As[r * b + k], Ds[k * b + c], acc);
+        out[(size_t)p * bb + e] = acc;
+    }
+}
+
 }  // namespace mgk

@@ -472,13 +472,17 @@ __global__ void gmres_begin_kernel(GmresDev s) {
     *s.hnext = beta;
 }
 
-// Back substitution H y = g over the j_used columns of this cycle.
-__global__ void gmres_solve_y_kernel(GmresDev s) {
+// Back substitution H y = g over the j_used columns of this cycle.  One warp: the inner sum over l > i is split
+// across the lanes (fixed lane -> l mapping and shuffle tree: deterministic).
+__global__ void __launch_bounds__(32) gmres_solve_y_kernel(GmresDev s) {
     const int ju = s.status[1];
+    const int lane = threadIdx.x;
     for (int i = ju - 1; i >= 0; --i) {
-        double t = s.g[i];
-        for (int l = i + 1; l < ju; ++l) t -= s.H[(size_t)l * (s.m + 1) + i] * s.y[l];
-        s.y[i] = t / s.H[(size_t)i * (s.m + 1) + i];
+        double t = 0.0;
+        for (int l = i + 1 + lane; l < ju; l += 32) t = fma(s.H[(size_t)l * (s.m + 1) + i], s.y[l], t);
+        t = warp_sum(t);
+        if (lane == 0) s.y[i] = (s.g[i] - t) / s.H[(size_t)i * (s.m + 1) + i];
+        __syncwarp();
     }
 }
 

@@ -88,6 +88,8 @@ struct mg_handle {
     double *red_partial = nullptr, *red_out = nullptr;
     unsigned *red_counter = nullptr;
     Gmres coarse, outer;
+    double *coarse_ahat = nullptr;       // A D^-1 of the coarsest level as one block-CSR matrix (fused coarse GMRES)
+    double *coarse_stage[2] = {nullptr, nullptr};  // unnormalised Arnoldi vectors between the SpMV and the CGS2 kernel
     cudaGraphExec_t coarse_graph = nullptr;
     int64_t coarse_graph_kernels = 0;
     bool capturing = false;
@@ -294,18 +296,6 @@ int pbj(mg_handle *h, const Level &L, const double *rin, double *dout, double c_
     a.done = done;
     return launch_bsr(h, L, a);
 }
-// vout = rin / *denom ; dout = Dinv vout   (TMA kernel only; vout may alias rin)
-int pbj_scaled(mg_handle *h, const Level &L, const double *rin, double *dout, const double *denom, double *vout,
-               const int *done) {
-    BsrArgs a{};
-    a.mode = MODE_PBJ;
-    a.rin = rin;
-    a.dout = dout;
-    a.c_z = 1.0;
-    a.done = done;
-    TmaExtra ex{nullptr, denom, vout};
-    return launch_bsr(h, L, a, ex);
-}
 int sweep(mg_handle *h, const Level &L, const double *vin, const double *rin, double *rout, double *x, double *dout,
           double c_d, double c_z, int flags) {
     BsrArgs a{};
@@ -485,10 +475,10 @@ int gmres_cycle_begin(mg_handle *h, Gmres &G, bool normalize = true) {
 // V[j+1] holds w = A M v_j: two classical Gram-Schmidt passes against V[0..j]; the tail of the second update
 // kernel does the Hessenberg column / Givens / stop test.  normalize: v_{j+1} = w / h_{j+1,j} here (otherwise the
 // caller folds the division into its next kernel).
-int gmres_orth(mg_handle *h, Gmres &G, int j, bool normalize = true) {
+int gmres_orth(mg_handle *h, Gmres &G, int j, bool normalize = true, double *w_override = nullptr) {
     KindScope scope(h, G.level, MG_KIND_ORTH);
     const int *done = G.dev.status;
-    double *w = G.V + (size_t)(j + 1) * G.stride;
+    double *w = w_override ? w_override : G.V + (size_t)(j + 1) * G.stride;
     if (G.fused_ok && h->opt.kernel_variant == 0) {
         OrthArgs oa{};
         oa.V = G.V;
@@ -529,7 +519,7 @@ int gmres_orth(mg_handle *h, Gmres &G, int j, bool normalize = true) {
 // y = H^-1 g ; out += sum_i y_i B_i  (B = Z for flexible, V otherwise)
 int gmres_cycle_end(mg_handle *h, Gmres &G, double *out) {
     KindScope scope(h, G.level, MG_KIND_ORTH);
-    LAUNCH(h, gmres_solve_y_kernel, 1, 1, 0, G.dev);
+    LAUNCH(h, gmres_solve_y_kernel, 1, 32, 0, G.dev);
     const int axpy_grid = (int)((G.n / 2 + 256) / 256);
     LAUNCH(h, axpy_multi_kernel, axpy_grid, 256, 0, G.flexible ? G.Z : G.V, G.stride, G.m, G.dev.status + 1, G.dev.y, 1.0,
            out, G.n, G.partial, G.counter + G.m + 1, (double *)nullptr, (const int *)nullptr, G.dev, -1);
@@ -544,20 +534,51 @@ int read_status(mg_handle *h, Gmres &G, int st[4]) {
 }
 
 // ------------------------------------------------------------------------------------------------ coarse solve
+// Fused coarse cycle (TMA kernel + fused CGS2): GMRES on the precomputed operator Ahat = A D^-1.  Two launches per
+// Arnoldi step.  S[0], S[1] alternate as the unnormalised Arnoldi vector: the SpMV of step j gathers S[j&1], writes
+// v_j = S[j&1] / h (the normalised basis vector) and S[(j+1)&1] = Ahat v_j; the CGS2 kernel orthogonalises
+// S[(j+1)&1] against V_0..V_j in place and leaves h_{j+1,j} for the next division.
+int coarse_cycle_enqueue_fused(mg_handle *h) {
+    Level &L = h->lev.back();
+    Gmres &G = h->coarse;
+    const int *done = G.dev.status;
+    MG(residual(h, L, L.rhs, L.x, h->coarse_stage[0], done));
+    {
+        KindScope scope(h, G.level, MG_KIND_ORTH);
+        LAUNCH(h, dot_multi_kernel, dim3(G.red_grid, 1), 256, 0, h->coarse_stage[0], (int64_t)0, h->coarse_stage[0], G.n, G.partial,
+               G.counter, G.dev.nrm2, done);
+        LAUNCH(h, gmres_begin_kernel, 1, 1, 0, G.dev);
+    }
+    Level Lhat = L;            // same pattern and partition, values A D^-1
+    Lhat.vals = h->coarse_ahat;
+    for (int j = 0; j < G.m; ++j) {
+        double *sj = h->coarse_stage[j & 1], *sn = h->coarse_stage[(j + 1) & 1];
+        BsrArgs a{};
+        a.mode = MODE_SPMV;
+        a.vin = sj;
+        a.out = sn;
+        a.done = done;
+        TmaExtra ex{nullptr, G.dev.hnext, G.V + (size_t)j * G.stride};
+        MG(launch_bsr(h, Lhat, a, ex));
+        MG(gmres_orth(h, G, j, false, sn));
+    }
+    CU(cudaMemsetAsync(L.d[1], 0, (size_t)L.nvec * sizeof(double), h->stream));
+    MG(gmres_cycle_end(h, G, L.d[1]));
+    MG(pbj(h, L, L.d[1], L.d[0], 1.0, L.x));  // e += D^-1 (V y)
+    return MG_OK;
+}
+
 int coarse_cycle_enqueue(mg_handle *h) {
     Level &L = h->lev.back();
     Gmres &G = h->coarse;
     const int *done = G.dev.status;
-    // TMA kernel: the division v_j = w / h_{j,j-1} rides in the PBJ apply that follows it (one launch, one pass)
-    const bool fused = h->tma_ready && h->opt.kernel_variant == 0 && L.part != nullptr;
+    if (h->coarse_ahat != nullptr && h->opt.kernel_variant == 0 && G.fused_ok) return coarse_cycle_enqueue_fused(h);
     MG(residual(h, L, L.rhs, L.x, G.V, done));
-    MG(gmres_cycle_begin(h, G, !fused));
+    MG(gmres_cycle_begin(h, G, true));
     for (int j = 0; j < G.m; ++j) {
-        double *vj = G.V + (size_t)j * G.stride;
-        if (fused) MG(pbj_scaled(h, L, vj, L.d[0], G.dev.hnext, vj, done));  // v_j /= h ; d0 = D^-1 v_j
-        else MG(pbj(h, L, vj, L.d[0], 1.0, nullptr, done));
+        MG(pbj(h, L, G.V + (size_t)j * G.stride, L.d[0], 1.0, nullptr, done));
         MG(spmv(h, L, L.d[0], G.V + (size_t)(j + 1) * G.stride, done));
-        MG(gmres_orth(h, G, j, !fused));
+        MG(gmres_orth(h, G, j, true));
     }
     CU(cudaMemsetAsync(L.d[1], 0, (size_t)L.nvec * sizeof(double), h->stream));
     MG(gmres_cycle_end(h, G, L.d[1]));
@@ -581,6 +602,15 @@ int coarse_solve_internal(mg_handle *h) {
         }
         MG(gmres_alloc(h, G, L.nvec, h->opt.coarse_restart, h->opt.coarse_maxit, false));
         G.level = L.index;
+        if (h->tma_ready && L.part != nullptr && G.fused_ok && h->coarse_ahat == nullptr && L.nnzb > 0) {
+            const int b = h->b;
+            MG(dalloc_t(h, &h->coarse_ahat, (size_t)L.nnzb * b * b));
+            MG(dalloc_t(h, &h->coarse_stage[0], (size_t)L.nvec + 2));
+            MG(dalloc_t(h, &h->coarse_stage[1], (size_t)L.nvec + 2));
+            LAUNCH(h, right_scale_blocks_kernel, (unsigned)L.nnzb, 256, sizeof(double) * 2 * b * b, L.col_idx, L.vals, L.dinv,
+                   h->coarse_ahat, b);
+            CU(cudaGetLastError());
+        }
     }
     CU(cudaMemsetAsync(L.x, 0, (size_t)L.nvec * sizeof(double), h->stream));
     MG(gmres_start(h, G, L.rhs, h->opt.coarse_rtol));
