@@ -113,6 +113,7 @@ class Options:
     coarse_fixed_sweeps: int = 8
     restart: int = 100
     maxit: int = 400
+    smoother: int = 0  # 0: PBJ-Chebyshev (north_star); 1: nu iterations of PBJ-preconditioned GMRES
 
 
 @dataclass
@@ -333,6 +334,24 @@ def fgmres(apply_A, apply_M, b: np.ndarray, x0=None, rtol: float = 1e-8, restart
 
 
 # ------------------------------------------------------------------------------------------------------------
+# NEXT-1  the paper's own level smoother: "one iteration of GMRES preconditioned with PBJ"
+# (App. B: ksp_type gmres, ksp_max_it 1, pc_type pbjacobi, ksp_norm_type none);
+# V(6,6) = the same with 6 iterations.  Reading (Q18): RIGHT preconditioning, so
+# that x_nu minimises the true residual ||rhs - A x|| over x_0 + D^-1 K_nu(A D^-1, r_0); no convergence test.
+# ------------------------------------------------------------------------------------------------------------
+def gmres_smoother(L: Level, rhs: np.ndarray, x0, nu: int) -> np.ndarray:
+    if nu <= 0:
+        return np.zeros(L.n) if x0 is None else x0.copy()
+    x, _, _, _ = fgmres(lambda v: spmv(L, v), lambda v: pbj_apply(L, v), rhs, x0, 0.0, nu, nu)
+    return x
+
+
+def smooth(H, L: Level, rhs: np.ndarray, x0, nu: int) -> np.ndarray:
+    """The level smoother selected by Options.smoother."""
+    return gmres_smoother(L, rhs, x0, nu) if H.opt.smoother == 1 else chebyshev(L, rhs, x0, nu)
+
+
+# ------------------------------------------------------------------------------------------------------------
 # 8c-K  coarsest-level solve, 8c-V  V-cycle (PAPER.md:63), setup
 # ------------------------------------------------------------------------------------------------------------
 def coarse_solve(H: Hierarchy, rhs: np.ndarray) -> np.ndarray:
@@ -354,11 +373,11 @@ def vcycle(H: Hierarchy, rhs: np.ndarray, lvl: int = 0) -> np.ndarray:
         return coarse_solve(H, rhs)
     L, o = H.levels[lvl], H.opt
     pphi = H.levels[lvl + 1].pphi
-    x = chebyshev(L, rhs, None, o.nu_pre)
+    x = smooth(H, L, rhs, None, o.nu_pre)
     res = rhs - spmv(L, x)
     e = vcycle(H, restrict(pphi, res), lvl + 1)
     x = x + prolong(pphi, e)
-    return chebyshev(L, rhs, x, o.nu_post)
+    return smooth(H, L, rhs, x, o.nu_post)
 
 
 def setup(row_ptr, col_idx, vals, b: int, n_pol: int, n_phi: int, levels: int, opt: Options = None) -> Hierarchy:
