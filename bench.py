@@ -43,7 +43,7 @@ RTOL = 1e-8
 # box): FGMRES / coarse-GMRES iteration counts of one C1 solve, as measured by this library on a B200 in round 1
 # (the oracle was never run to convergence at this size: hours of CPU time).  Used ONLY to scale a measured
 # oracle GB/s to a solve; never an input or an expected value of any parity test.
-REFERENCE_COUNTS = {"C1": dict(outer_iters=186, coarse_iters=903027), "C0": dict(outer_iters=40, coarse_iters=40000)}
+REFERENCE_COUNTS = {"C1": dict(outer_iters=186, coarse_iters=664740), "C0": dict(outer_iters=40, coarse_iters=40000)}
 
 
 def log(*a):
@@ -212,7 +212,7 @@ def reference_arm(args):
     oracle_mg.build()
     w = make_workload(args.workload)
     sizes = oracle_level_sizes(w)
-    opt = dict(nu_pre=2, nu_post=2, restart=100, coarse_restart=50)
+    opt = dict(nu_pre=2, nu_post=2, restart=100, coarse_restart=100)
     counts = REFERENCE_COUNTS.get(args.workload, REFERENCE_COUNTS["C1"])
     total_bytes = solve_bytes_from_counts(sizes, counts["outer_iters"], counts["coarse_iters"], opt)
     per_step = max(0.05, min(args.cpu_seconds, 150.0 / max(1, args.steps + args.warmup)))

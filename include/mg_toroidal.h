@@ -65,7 +65,7 @@ typedef struct mg_options {
     int coarse_mode;         /* 0: PBJ-GMRES(coarse_restart) to coarse_rtol (default);
                                 1: coarse_fixed_sweeps Chebyshev-PBJ sweeps (a fixed polynomial: parity mode) */
     double coarse_rtol;      /* default 1e-10 (configs[1]) */
-    int coarse_restart, coarse_maxit, coarse_fixed_sweeps; /* defaults 50, 20000, 8 */
+    int coarse_restart, coarse_maxit, coarse_fixed_sweeps; /* defaults 100, 20000, 8 (restart: DESIGN.md Q9) */
     int restart, maxit;      /* outer FGMRES restart length and iteration cap; defaults 100, 400
                                 (paper: 200 / 200) */
     int block_layout;        /* 0: row-major b x b blocks (only layout supported) */
@@ -73,6 +73,9 @@ typedef struct mg_options {
     int kernel_variant;      /* launch mechanics only (same arithmetic up to summation order): 0 (default) the
                                 persistent TMA-ring block-CSR kernel where it exists (b = 36), 1 the one-CTA-per-row
                                 128-bit-load kernel for every b (kept for A/B measurement) */
+    int smoother;            /* 0 (default): PBJ-Chebyshev (BASELINE.json north_star); 1: nu iterations of right-PBJ-
+                                preconditioned GMRES without a convergence test -- the paper's own level smoother,
+                                "one iteration of GMRES preconditioned with PBJ", V(1,1) / V(6,6) */
     mg_alloc_fn alloc;       /* NULL => cudaMalloc */
     mg_free_fn free;         /* NULL => cudaFree */
     void *alloc_ctx;

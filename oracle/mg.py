@@ -108,7 +108,7 @@ class Options:
     eig_iters: int = 20
     coarse_mode: int = 0  # 0: PBJ-GMRES to coarse_rtol; 1: coarse_fixed_sweeps of Chebyshev-PBJ
     coarse_rtol: float = 1e-10
-    coarse_restart: int = 50
+    coarse_restart: int = 100
     coarse_maxit: int = 20000
     coarse_fixed_sweeps: int = 8
     restart: int = 100

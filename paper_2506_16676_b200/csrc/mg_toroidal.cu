@@ -88,6 +88,7 @@ struct mg_handle {
     double *red_partial = nullptr, *red_out = nullptr;
     unsigned *red_counter = nullptr;
     Gmres coarse, outer;
+    std::vector<Gmres> smooth_g;         // per level: Arnoldi engine of the GMRES-PBJ smoother (opt.smoother = 1)
     double *coarse_ahat = nullptr;       // A D^-1 of the coarsest level as one block-CSR matrix (fused coarse GMRES)
     double *coarse_stage[2] = {nullptr, nullptr};  // unnormalised Arnoldi vectors between the SpMV and the CGS2 kernel
     cudaGraphExec_t coarse_graph = nullptr;
@@ -660,6 +661,37 @@ int coarse_solve_internal(mg_handle *h) {
     return MG_OK;
 }
 
+// ------------------------------------------------------------------------------------------------ GMRES smoother
+// The paper's level smoother (App. B 421-424): nu iterations of GMRES preconditioned (on the right) with
+// PBJ, no convergence test, no restart: x <- argmin ||rhs - A x|| over x0 + D^-1 K_nu(A D^-1, r0).  Everything stays on
+// the device: the Arnoldi/Givens state is GmresDev, the tolerance is 0, nothing is read back.
+int gmres_smooth(mg_handle *h, Level &L, const double *rhs, double *x, int nu, bool zero_guess) {
+    const size_t bytes = (size_t)L.nvec * sizeof(double);
+    if (zero_guess) CU(cudaMemsetAsync(x, 0, bytes, h->stream));
+    if (nu <= 0 || L.nvec == 0) return MG_OK;
+    if ((int)h->smooth_g.size() != h->n_levels) h->smooth_g.resize(h->n_levels);
+    Gmres &G = h->smooth_g[L.index];
+    if (!G.ready || G.m < nu) {
+        const int m = std::max(nu, std::max(h->opt.nu_pre, h->opt.nu_post));
+        MG(gmres_alloc(h, G, L.nvec, m, m, false));  // maxit = m: the stop flag can only rise after the last step
+        G.level = L.index;
+    }
+    const int *done = G.dev.status;
+    MG(gmres_start(h, G, rhs, 0.0));
+    if (zero_guess) CU(cudaMemcpyAsync(G.V, rhs, bytes, cudaMemcpyDeviceToDevice, h->stream));
+    else MG(residual(h, L, rhs, x, G.V));
+    MG(gmres_cycle_begin(h, G, true));
+    for (int j = 0; j < nu; ++j) {
+        MG(pbj(h, L, G.V + (size_t)j * G.stride, L.d[0], 1.0, nullptr, done));
+        MG(spmv(h, L, L.d[0], G.V + (size_t)(j + 1) * G.stride, done));
+        MG(gmres_orth(h, G, j, true));
+    }
+    CU(cudaMemsetAsync(L.d[1], 0, bytes, h->stream));
+    MG(gmres_cycle_end(h, G, L.d[1]));
+    MG(pbj(h, L, L.d[1], L.d[0], 1.0, x));  // x += D^-1 (V y)
+    return MG_OK;
+}
+
 // ------------------------------------------------------------------------------------------------ V-cycle
 int vcycle_internal(mg_handle *h, const double *r, double *z) {
     const int Lc = h->n_levels - 1;
@@ -670,19 +702,30 @@ int vcycle_internal(mg_handle *h, const double *r, double *z) {
         CU(cudaMemcpyAsync(z, L.x, (size_t)L.nvec * sizeof(double), cudaMemcpyDeviceToDevice, h->stream));
         return MG_OK;
     }
+    const bool gsm = (h->opt.smoother == 1);
     for (int l = 0; l < Lc; ++l) {
         Level &L = h->lev[l];
         const double *rhs = (l == 0) ? r : L.rhs;
         double *x = (l == 0) ? z : L.x;
-        MG(presmooth(h, L, rhs, x, h->opt.nu_pre));
+        if (gsm) {
+            MG(gmres_smooth(h, L, rhs, x, h->opt.nu_pre, true));
+            MG(residual(h, L, rhs, x, L.r));
+        } else {
+            MG(presmooth(h, L, rhs, x, h->opt.nu_pre));
+        }
         MG(restrict_to(h, l, L.r, h->lev[l + 1].rhs));
     }
     MG(coarse_solve_internal(h));
     for (int l = Lc - 1; l >= 0; --l) {
         Level &L = h->lev[l];
         double *x = (l == 0) ? z : L.x;
-        MG(prolong_add(h, l, h->lev[l + 1].x, x, h->opt.nu_post > 0 ? L.pe : nullptr));
-        MG(postsmooth(h, L, L.pe, x, h->opt.nu_post));
+        if (gsm) {
+            MG(prolong_add(h, l, h->lev[l + 1].x, x, nullptr));
+            MG(gmres_smooth(h, L, (l == 0) ? r : L.rhs, x, h->opt.nu_post, false));
+        } else {
+            MG(prolong_add(h, l, h->lev[l + 1].x, x, h->opt.nu_post > 0 ? L.pe : nullptr));
+            MG(postsmooth(h, L, L.pe, x, h->opt.nu_post));
+        }
     }
     return MG_OK;
 }
@@ -866,7 +909,7 @@ int mg_options_default(mg_options *o) {
     o->eig_iters = 20;
     o->coarse_mode = 0;
     o->coarse_rtol = 1e-10;
-    o->coarse_restart = 50;
+    o->coarse_restart = 100;
     o->coarse_maxit = 20000;
     o->coarse_fixed_sweeps = 8;
     o->restart = 100;
@@ -874,6 +917,7 @@ int mg_options_default(mg_options *o) {
     o->block_layout = 0;
     o->use_graphs = 1;
     o->kernel_variant = 0;
+    o->smoother = 0;
     return MG_OK;
 }
 
@@ -884,6 +928,7 @@ static int validate_options(const mg_options &o) {
     if (o.coarse_restart < 1 || o.coarse_maxit < 1 || o.coarse_fixed_sweeps < 0) return MG_EINVAL;
     if (o.restart < 1 || o.maxit < 1 || o.block_layout != 0) return MG_EINVAL;
     if (o.kernel_variant < 0 || o.kernel_variant > 1) return MG_EINVAL;
+    if (o.smoother < 0 || o.smoother > 1) return MG_EINVAL;
     return MG_OK;
 }
 
@@ -1128,6 +1173,7 @@ int mg_pbj_apply(mg_handle *h, int level, const double *r, double *z) {
 int mg_smooth(mg_handle *h, int level, const double *rhs, double *x, int nu, int zero_guess) {
     if (!level_ok(h, level) || !rhs || !x || nu < 0 || rhs == x) return MG_EINVAL;
     Level &L = h->lev[level];
+    if (h->opt.smoother == 1) return gmres_smooth(h, L, rhs, x, nu, zero_guess != 0);
     if (zero_guess) return presmooth(h, L, rhs, x, nu);
     if (nu == 0) return MG_OK;
     const size_t bytes = (size_t)L.nvec * sizeof(double);

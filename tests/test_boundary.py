@@ -43,7 +43,7 @@ def test_options_default_values():
     o = binding.options_default()
     assert (o.nu_pre, o.nu_post) == (2, 2)                      # "2 Chebyshev-PBJ sweeps", configs[0]
     assert (o.cheb_lo, o.cheb_hi, o.eig_iters) == (0.1, 1.1, 20)
-    assert (o.coarse_mode, o.coarse_rtol, o.coarse_restart, o.coarse_maxit) == (0, 1e-10, 50, 20000)
+    assert (o.coarse_mode, o.coarse_rtol, o.coarse_restart, o.coarse_maxit) == (0, 1e-10, 100, 20000)
     assert (o.restart, o.maxit) == (100, 400)
     assert binding.lib().mg_options_default(None) == binding.MG_EINVAL
 

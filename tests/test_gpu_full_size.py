@@ -90,7 +90,7 @@ def test_c1_first_outer_iterations_pinned_mode(c1):
 
 
 def test_c1_default_mode_properties(c1):
-    """The configuration bench.py times (PBJ-GMRES(50) coarse solve to 1e-10, CUDA graph), cut after 2 outer
+    """The configuration bench.py times (PBJ-GMRES(100) coarse solve to 1e-10, CUDA graph), cut after 2 outer
     iterations: estimate == true residual; and the coarsest-level solve meets its tolerance on the oracle's matrix."""
     w, H, s = c1
     s.update_options(coarse_mode=0, maxit=2)

@@ -60,7 +60,7 @@ def test_vcycle_default_mode_residual_sense(case):
 @pytest.mark.parametrize("case", ["b12-3lev", "b6-4lev", "b5-generic-to-1-plane"])
 @pytest.mark.parametrize("graphs", [1, 0])
 def test_coarse_solve(case, graphs):
-    """PBJ-GMRES(50) to 1e-10 on the coarsest level: both reach the tolerance; the solutions agree to
+    """PBJ-GMRES(100) to 1e-10 on the coarsest level: both reach the tolerance; the solutions agree to
     cond * rtol.  The inner iteration COUNT is not a parity quantity (north_star's +-1 is for the outer FGMRES):
     a restarted GMRES that needs ~60 restart cycles near stagnation amplifies the rounding difference between
     CGS2 (device) and MGS (oracle) -- cf. PAPER.md:170, CPU and GPU counts of the same solver differ -- so the
