@@ -261,7 +261,12 @@ def cuda_arm(args):
     rp, ci, va = binding.upload(w, dev)
     torch.cuda.synchronize()
     t0 = time.perf_counter()
-    s = binding.Solver(rp, ci, va, w.b, w.n_pol, w.n_phi, w.levels)
+    extra = {}
+    if args.smoother == "gmres":
+        extra["smoother"] = 1
+    if args.nu > 0:
+        extra.update(nu_pre=args.nu, nu_post=args.nu)
+    s = binding.Solver(rp, ci, va, w.b, w.n_pol, w.n_phi, w.levels, **extra)
     torch.cuda.synchronize()
     setup_s = time.perf_counter() - t0
     if args.max_outer > 0:
@@ -368,7 +373,7 @@ def cuda_arm(args):
         vc_ms = v0.elapsed_time(v1) / 5
         vc_bytes = vcycle_bytes(sizes, opt["nu_pre"], opt["nu_post"], coarse_sweeps=s.opt.coarse_fixed_sweeps)
         solve_bytes = solve_bytes_from_counts(sizes, info["iters"], info["coarse_iters_total"], opt)
-        vcycle_roof = {
+        vcycle_roof = None if args.smoother == "gmres" else {   # the byte model below is the Chebyshev cycle's
             "pinned_coarse_mode": {"ms": vc_ms, "bytes": vc_bytes, "GBps": vc_bytes / vc_ms / 1e6,
                                    "frac_of_measured_peak": vc_bytes / vc_ms / 1e6 / peak, "frac_of_8TBs_nominal": vc_bytes / vc_ms / 1e6 / 8000.0},
             "complete_outer_iteration": {"ms": 1e3 * t_dev / max(1, info["iters"]), "bytes": solve_bytes / max(1, info["iters"]),
@@ -394,7 +399,7 @@ def cuda_arm(args):
                 "ms_per_step": 1e3 * t_dev, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
                 "config": {"workload": w.name, "n_pol": w.n_pol, "n_phi": w.n_phi, "b": w.b, "levels": w.levels,
-                           "unknowns": n, "nnzb": w.nnzb, "rtol": RTOL, "cycle": f"V({opt['nu_pre']},{opt['nu_post']}) PBJ-Chebyshev",
+                           "unknowns": n, "nnzb": w.nnzb, "rtol": RTOL, "cycle": f"V({opt['nu_pre']},{opt['nu_post']}) " + ("PBJ-GMRES smoother (the paper's, PAPER.md:95)" if args.smoother == "gmres" else "PBJ-Chebyshev"),
                            "coarsest": f"PBJ-GMRES({opt['coarse_restart']}) to {opt['coarse_rtol']:g}", "fgmres_restart": opt["restart"],
                            "parallelism": "replicas only" if world > 1 else "1 GPU", "setup_s": setup_s,
                            "l2": "inputs larger than L2 (every level's matrix >= 0.5 GB vs 126 MB L2)" if sizes[-1].matrix_bytes > 2.6e8
@@ -441,6 +446,9 @@ def main():
     ap.add_argument("--max-outer", type=int, default=0,
                     help="profiling aid (ncu launch lists): cap the outer FGMRES iterations of every solve; the line is then "
                          "marked \"truncated\": true and is NOT a bench value")
+    ap.add_argument("--smoother", choices=["chebyshev", "gmres"], default="chebyshev",
+                    help="level smoother: PBJ-Chebyshev (default, the metric's configuration) or the paper's PBJ-GMRES (NEXT-1)")
+    ap.add_argument("--nu", type=int, default=0, help="smoothing steps pre and post (default: the library's 2)")
     ap.add_argument("--warmup-outer", type=int, default=4,
                     help="outer FGMRES iterations of each warm-up step (default 4, about 2.5 s on C1); 0 = complete solves")
     ap.add_argument("--kernel-sweep", nargs="*", default=None, metavar="TOKEN",
