@@ -111,6 +111,17 @@ int mg_setup(mg_handle **h, const int64_t *row_ptr, const int32_t *col_idx, cons
  * rebuilding the hierarchy; alloc/free/eig_iters/block_layout are ignored. */
 int mg_update_options(mg_handle *h, const mg_options *opt);
 
+/* Lagged preconditioner ("one new Jacobian per time step ... the preconditioner
+ * is lagged, refreshed every `refresh period` steps"; refresh cost: Table 4).
+ * mg_update_values -- REFRESH: new fine-level values with the SAME pattern (device pointer, borrowed from now on in
+ *   place of the old one): recomputes the block inverses, the Chebyshev bounds and the Galerkin operators into the
+ *   existing patterns and allocations (no symbolic phase).  Also resets the solve operator to these values.
+ *   Errors: MG_EINVAL, MG_ESINGULAR, MG_ECUDA.  Synchronises the stream.
+ * mg_set_operator -- LAG: mg_solve iterates on A_new = (level-0 pattern, `vals`) while the V-cycle keeps the
+ *   hierarchy of the last setup/refresh.  vals: device pointer, borrowed; NULL = back to the hierarchy's own matrix. */
+int mg_update_values(mg_handle *h, const double *vals);
+int mg_set_operator(mg_handle *h, const double *vals);
+
 /* mg_vcycle -- z = M(r): one V(nu_pre,nu_post) cycle from a zero guess.  r, z: level-0
  * vectors; r is not modified, z is overwritten.  Asynchronous in coarse_mode 1. */
 int mg_vcycle(mg_handle *h, const double *r, double *z);

@@ -38,6 +38,8 @@ SYMBOLS = {
     "mg_options_default": (_I, [C.POINTER(mg_options)]),
     "mg_setup": (_I, [C.POINTER(_VP), _VP, _VP, _VP, _I, _I, _I, _I, C.POINTER(mg_options), _VP]),
     "mg_update_options": (_I, [_VP, C.POINTER(mg_options)]),
+    "mg_update_values": (_I, [_VP, _VP]),
+    "mg_set_operator": (_I, [_VP, _VP]),
     "mg_vcycle": (_I, [_VP, _VP, _VP]),
     "mg_solve": (_I, [_VP, _VP, _VP, _D, _I, C.POINTER(mg_solve_info)]),
     "mg_solve_host": (_I, [_VP, _VP, _VP, _D, _I, C.POINTER(mg_solve_info)]),
@@ -171,6 +173,19 @@ class Solver:
         _chk(lib().mg_update_options(self._h, C.byref(self.opt)), "mg_update_options")
 
     # ---- the C ABI -----------------------------------------------------------------------------------------
+    def update_values(self, vals):
+        """Refresh: new fine values (same pattern); the library borrows ``vals`` from now on."""
+        import torch
+        _chk(lib().mg_update_values(self._h, _ptr(vals, torch.float64)), "mg_update_values")
+        self.vals = vals
+        self._op_vals = None
+
+    def set_operator(self, vals=None):
+        """Lag: solve with (pattern, ``vals``) while the V-cycle keeps the old hierarchy; None = hierarchy's matrix."""
+        import torch
+        _chk(lib().mg_set_operator(self._h, _ptr(vals, torch.float64) if vals is not None else None), "mg_set_operator")
+        self._op_vals = vals
+
     def vcycle(self, r, z=None):
         import torch
         z = self.new() if z is None else z

@@ -30,6 +30,8 @@ struct Level {
     const int32_t *col_idx = nullptr;
     const double *vals = nullptr;
     int64_t *diag_pos = nullptr;
+    int64_t *row_of_block = nullptr;  // coarse levels: block row of every stored block (Galerkin numeric phase)
+    unsigned long long *err_flag = nullptr;  // device flag of the batched inverse (first singular block, or ~0)
     double *dinv = nullptr;
     int64_t *part = nullptr;  // TMA kernel: first block row of each persistent CTA (tma_grid + 1 entries)
     int tma_grid = 0;
@@ -89,6 +91,7 @@ struct mg_handle {
     unsigned *red_counter = nullptr;
     Gmres coarse, outer;
     std::vector<Gmres> smooth_g;         // per level: Arnoldi engine of the GMRES-PBJ smoother (opt.smoother = 1)
+    const double *outer_vals = nullptr;  // values of the operator FGMRES solves with (mg_set_operator); NULL = level 0's
     double *coarse_ahat = nullptr;       // A D^-1 of the coarsest level as one block-CSR matrix (fused coarse GMRES)
     double *coarse_stage[2] = {nullptr, nullptr};  // unnormalised Arnoldi vectors between the SpMV and the CGS2 kernel
     cudaGraphExec_t coarse_graph = nullptr;
@@ -587,6 +590,17 @@ int coarse_cycle_enqueue(mg_handle *h) {
     return MG_OK;
 }
 
+// Ahat = A D^-1 of the coarsest level (values only; the pattern is A's).
+int refresh_coarse_ahat(mg_handle *h) {
+    Level &L = h->lev.back();
+    if (h->coarse_ahat == nullptr || L.nnzb == 0) return MG_OK;
+    const int b = h->b;
+    LAUNCH(h, right_scale_blocks_kernel, (unsigned)L.nnzb, 256, sizeof(double) * 2 * b * b, L.col_idx, L.vals, L.dinv,
+           h->coarse_ahat, b);
+    CU(cudaGetLastError());
+    return MG_OK;
+}
+
 // Solve A_{L-1} x = rhs on the coarsest level's own buffers (L.rhs -> L.x), zero guess.
 int coarse_solve_internal(mg_handle *h) {
     Level &L = h->lev.back();
@@ -608,9 +622,7 @@ int coarse_solve_internal(mg_handle *h) {
             MG(dalloc_t(h, &h->coarse_ahat, (size_t)L.nnzb * b * b));
             MG(dalloc_t(h, &h->coarse_stage[0], (size_t)L.nvec + 2));
             MG(dalloc_t(h, &h->coarse_stage[1], (size_t)L.nvec + 2));
-            LAUNCH(h, right_scale_blocks_kernel, (unsigned)L.nnzb, 256, sizeof(double) * 2 * b * b, L.col_idx, L.vals, L.dinv,
-                   h->coarse_ahat, b);
-            CU(cudaGetLastError());
+            MG(refresh_coarse_ahat(h));
         }
     }
     CU(cudaMemsetAsync(L.x, 0, (size_t)L.nvec * sizeof(double), h->stream));
@@ -824,28 +836,51 @@ int alloc_level_vectors(mg_handle *h, Level &L) {
     return MG_OK;
 }
 
+int invert_level_blocks(mg_handle *h, Level &L);
+
 int setup_level_pbj(mg_handle *h, Level &L) {
     const int b = h->b;
     MG(dalloc_t(h, &L.diag_pos, (size_t)L.n_brows));
     unsigned long long *err = nullptr;
-    MG(dalloc_t(h, &err, 3));
-    CU(cudaMemsetAsync(err, 0xff, 3 * sizeof(unsigned long long), h->stream));
+    MG(dalloc_t(h, &err, 2));
+    CU(cudaMemsetAsync(err, 0xff, 2 * sizeof(unsigned long long), h->stream));
     LAUNCH(h, check_pattern_kernel, grid_for(L.n_brows, 256, 1 << 30), 256, 0, L.row_ptr, L.col_idx, L.n_brows, L.diag_pos,
            err, err + 1);
-    unsigned long long herr[3];
+    unsigned long long herr[2];
     CU(cudaMemcpyAsync(herr, err, sizeof(herr), cudaMemcpyDeviceToHost, h->stream));
     CU(cudaStreamSynchronize(h->stream));
     if (herr[0] != ~0ull) return MG_EINVAL;
     if (herr[1] != ~0ull) return MG_ESINGULAR;
     MG(dalloc_t(h, &L.dinv, (size_t)L.n_brows * b * b));
+    MG(dalloc_t(h, &L.err_flag, 1));
+    return invert_level_blocks(h, L);
+}
+
+// Batched inverse of the diagonal blocks of one level into L.dinv; MG_ESINGULAR on a zero pivot.
+int invert_level_blocks(mg_handle *h, Level &L) {
+    const int b = h->b;
+    unsigned long long *err = L.err_flag;
+    unsigned long long herr[1];
+    CU(cudaMemsetAsync(err, 0xff, sizeof(unsigned long long), h->stream));
     const size_t smem = sizeof(double) * (size_t)(2 * b * b + b);
     if (smem > 48 * 1024)
         CU(cudaFuncSetAttribute(invert_blocks_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    if (L.n_brows > 0) LAUNCH(h, invert_blocks_kernel, (unsigned)L.n_brows, 128, smem, L.vals, L.diag_pos, b, L.dinv, err + 2);
+    if (L.n_brows > 0) LAUNCH(h, invert_blocks_kernel, (unsigned)L.n_brows, 128, smem, L.vals, L.diag_pos, b, L.dinv, err);
     CU(cudaGetLastError());
     CU(cudaMemcpyAsync(herr, err, sizeof(herr), cudaMemcpyDeviceToHost, h->stream));
     CU(cudaStreamSynchronize(h->stream));
-    if (herr[2] != ~0ull) return MG_ESINGULAR;
+    if (herr[0] != ~0ull) return MG_ESINGULAR;
+    return MG_OK;
+}
+
+// Numeric phase of A_{l+1} = P^T A_l P into the existing pattern of level l+1 (mg_setup and mg_update_values).
+int galerkin_numeric(mg_handle *h, int l) {
+    Level &F = h->lev[l];
+    Level &C = h->lev[l + 1];
+    if (C.nnzb > 0)
+        LAUNCH(h, galerkin_numeric_kernel, (unsigned)C.nnzb, 128, 0, F.row_ptr, F.col_idx, F.vals, C.row_of_block, C.col_idx,
+               const_cast<double *>(C.vals), h->n_pol, F.n_phi, h->b);
+    CU(cudaGetLastError());
     return MG_OK;
 }
 
@@ -872,24 +907,16 @@ int build_coarse_level(mg_handle *h, int l) {
     MG(dalloc_t(h, &d_rp, (size_t)C.n_brows + 1));
     MG(dalloc_t(h, &d_ci, (size_t)C.nnzb));
     MG(dalloc_t(h, &d_v, (size_t)C.nnzb * b * b));
-    cudaError_t e = cudaMalloc(&d_rob, sizeof(int64_t) * std::max<int64_t>(C.nnzb, 1));
-    if (e != cudaSuccess) {
-        cudaGetLastError();
-        return MG_ENOMEM;
-    }
+    MG(dalloc_t(h, &d_rob, (size_t)std::max<int64_t>(C.nnzb, 1)));
     CU(cudaMemcpyAsync(d_rp, C.h_row_ptr.data(), sizeof(int64_t) * (C.n_brows + 1), cudaMemcpyHostToDevice, h->stream));
     CU(cudaMemcpyAsync(d_ci, C.h_col_idx.data(), sizeof(int32_t) * C.nnzb, cudaMemcpyHostToDevice, h->stream));
     CU(cudaMemcpyAsync(d_rob, crow_of_block.data(), sizeof(int64_t) * C.nnzb, cudaMemcpyHostToDevice, h->stream));
-    if (C.nnzb > 0)
-        LAUNCH(h, galerkin_numeric_kernel, (unsigned)C.nnzb, 128, 0, F.row_ptr, F.col_idx, F.vals, d_rob, d_ci, d_v, h->n_pol,
-               F.n_phi, b);
-    CU(cudaGetLastError());
-    CU(cudaStreamSynchronize(h->stream));
-    cudaFree(d_rob);
+    CU(cudaStreamSynchronize(h->stream));  // crow_of_block is a local
     C.row_ptr = d_rp;
     C.col_idx = d_ci;
     C.vals = d_v;
-    return MG_OK;
+    C.row_of_block = d_rob;
+    return galerkin_numeric(h, l);
 }
 
 bool level_ok(mg_handle *h, int level) { return h && level >= 0 && level < h->n_levels; }
@@ -1058,6 +1085,28 @@ int mg_update_options(mg_handle *h, const mg_options *opt) {
     return MG_OK;
 }
 
+int mg_update_values(mg_handle *h, const double *vals) {
+    if (!h || !vals) return MG_EINVAL;
+    h->lev[0].vals = vals;
+    h->outer_vals = nullptr;
+    for (int l = 0; l < h->n_levels; ++l) {
+        Level &L = h->lev[l];
+        MG(invert_level_blocks(h, L));
+        MG(power_rho(h, L, h->opt.eig_iters, &L.rho_est));
+        set_bounds(h, L);
+        if (l + 1 < h->n_levels) MG(galerkin_numeric(h, l));
+    }
+    MG(refresh_coarse_ahat(h));
+    CU(cudaStreamSynchronize(h->stream));
+    return MG_OK;
+}
+
+int mg_set_operator(mg_handle *h, const double *vals) {
+    if (!h) return MG_EINVAL;
+    h->outer_vals = vals;
+    return MG_OK;
+}
+
 int mg_vcycle(mg_handle *h, const double *r, double *z) {
     if (!h || !r || !z || r == z) return MG_EINVAL;
     return vcycle_internal(h, r, z);
@@ -1065,7 +1114,10 @@ int mg_vcycle(mg_handle *h, const double *r, double *z) {
 
 int mg_solve(mg_handle *h, const double *rhs, double *x, double rtol, int x_is_initial_guess, mg_solve_info *info) {
     if (!h || !rhs || !x || rhs == x || !(rtol > 0.0)) return MG_EINVAL;
-    Level &L = h->lev[0];
+    Level L = h->lev[0];  // the operator of the Krylov iteration: level 0's pattern with the current operator values
+    L.h_row_ptr.clear();
+    L.h_col_idx.clear();
+    if (h->outer_vals != nullptr) L.vals = h->outer_vals;
     Gmres &G = h->outer;
     const int64_t n = L.nvec;
     const size_t bytes = (size_t)n * sizeof(double);
