@@ -47,8 +47,8 @@ struct TmaCfg {
 // extra arguments of the TMA kernel (the common ones are BsrArgs)
 struct TmaExtra {
     const int64_t *part;      // [gridDim.x + 1] first block row of every CTA (nullptr: uniform split, implicit diagonal)
-    const double *scale_div;  // PBJ and SPMV modes, optional: the input vector is (rin | vin) / *scale_div
-    double *vout;             // PBJ and SPMV modes, optional: vout_I = (rin_I | vin_I) / *scale_div (PBJ: may alias rin)
+    const double *scale_div;  // SPMV mode, optional: the input vector is vin / *scale_div (out = A vin / *scale_div)
+    double *vout;             // SPMV mode, optional: vout_I = vin_I / *scale_div (the normalised input; vout != vin)
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -206,7 +206,7 @@ __global__ void __launch_bounds__(TmaCfg::THREADS, 1) bsr_tma_kernel(const BsrAr
     double *vec = sVec + g * C::VECPAD;
     double inv_scale = 1.0;
     const bool spmv_scaled = (a.mode == MODE_SPMV) && ex.scale_div != nullptr;
-    if ((diag || spmv_scaled) && ex.scale_div != nullptr) inv_scale = 1.0 / *ex.scale_div;
+    if (spmv_scaled) inv_scale = 1.0 / *ex.scale_div;
 
     int seen = 0;  // last value read from `issued`
     int64_t I = R0 + g;
@@ -229,7 +229,7 @@ __global__ void __launch_bounds__(TmaCfg::THREADS, 1) bsr_tma_kernel(const BsrAr
 #pragma unroll
         for (int c = 0; c < C::SEGL; ++c) dreg[c] = 0.0;
         if (active) {
-            if (a.mode == MODE_RESID || sweep || (diag && ex.vout != nullptr)) rin_v = a.rin[gi];
+            if (a.mode == MODE_RESID || sweep) rin_v = a.rin[gi];
             if (sweep || (spmv_scaled && ex.vout != nullptr)) dold = a.vin[gi];
             if (touch_x && !(flags & F_SET_X)) xold = a.x[gi];
             if (need_d) {
@@ -281,10 +281,9 @@ __global__ void __launch_bounds__(TmaCfg::THREADS, 1) bsr_tma_kernel(const BsrAr
         } else if (a.mode == MODE_RESID) {
             if (writer) a.out[gi] = rin_v - acc;
         } else if (diag) {
-            const double dnew = a.c_z * (acc * inv_scale);
+            const double dnew = a.c_z * acc;
             if (writer) {
                 a.dout[gi] = dnew;
-                if (ex.vout != nullptr) ex.vout[gi] = rin_v * inv_scale;
                 if (flags & F_FINAL_X) a.x[gi] = xold + dnew;
             }
         } else {
