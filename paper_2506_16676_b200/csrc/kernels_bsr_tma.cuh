@@ -46,7 +46,12 @@ struct TmaCfg {
 
 // extra arguments of the TMA kernel (the common ones are BsrArgs)
 struct TmaExtra {
-    const int64_t *part;      // [gridDim.x + 1] first block row of every CTA (nullptr: uniform split, implicit diagonal)
+    const int64_t *part;      // [2*(gridDim.x + 1)] per CTA k: {first block P_k, first OWNED block row Ra_k} (nullptr: uniform
+                              // split of the implicit block-diagonal matrix).  A CTA owns the rows that START in [P_k, P_k+1).
+                              // When P_k falls inside a row (balanced split), CTA k multiplies the row's remaining blocks first
+                              // and hands the 36 partial sums to the owner CTA k-1 through frag_part / frag_flag.
+    double *frag_part;        // [gridDim.x][36]
+    int *frag_flag;           // [gridDim.x] zero-initialised; set by the fragment's CTA, cleared by the owner
     const double *scale_div;  // SPMV mode, optional: the input vector is vin / *scale_div (out = A vin / *scale_div)
     double *vout;             // SPMV mode, optional: vout_I = vin_I / *scale_div (the normalised input; vout != vin)
 };
@@ -100,12 +105,25 @@ __device__ __forceinline__ void group_bar(int g) {
 
 // part[k] = first block row I with row_ptr[I] >= k * nnzb / nparts (k = 0..nparts; part[nparts] = n_brows):
 // contiguous row ranges holding (nearly) equal numbers of blocks.
+// max over block rows of the number of stored blocks
+__global__ void max_row_blocks_kernel(const int64_t *__restrict__ row_ptr, const int64_t n_brows, int *__restrict__ out) {
+    int m = 0;
+    for (int64_t I = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; I < n_brows; I += (int64_t)gridDim.x * blockDim.x)
+        m = max(m, (int)(row_ptr[I + 1] - row_ptr[I]));
+    for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0 && m > 0) atomicMax(out, m);
+}
+
+// split != 0: P_k = k*nnzb/nparts exactly (equal block counts; a row may straddle two CTAs); split == 0: P_k is moved up to
+// the next row start (row-aligned ranges, +-1 row of imbalance).  part[2k] = P_k, part[2k+1] = Ra_k = first row with
+// row_ptr >= P_k.
 __global__ void partition_rows_kernel(const int64_t *__restrict__ row_ptr, const int64_t n_brows, const int64_t nnzb,
-                                      const int nparts, int64_t *__restrict__ part) {
+                                      const int nparts, const int split, int64_t *__restrict__ part) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k > nparts) return;
     if (k == nparts) {
-        part[k] = n_brows;
+        part[2 * k] = nnzb;
+        part[2 * k + 1] = n_brows;
         return;
     }
     const int64_t target = (int64_t)(((__int128)nnzb * k) / nparts);
@@ -114,7 +132,8 @@ __global__ void partition_rows_kernel(const int64_t *__restrict__ row_ptr, const
         const int64_t mid = (lo + hi) >> 1;
         if (row_ptr[mid] >= target) hi = mid; else lo = mid + 1;
     }
-    part[k] = lo;
+    part[2 * k] = split ? target : row_ptr[lo];
+    part[2 * k + 1] = lo;
 }
 
 __global__ void __launch_bounds__(TmaCfg::THREADS, 1) bsr_tma_kernel(const BsrArgs a, const TmaExtra ex) {
@@ -136,17 +155,22 @@ __global__ void __launch_bounds__(TmaCfg::THREADS, 1) bsr_tma_kernel(const BsrAr
     const bool diag = (a.mode == MODE_PBJ);             // implicit block-diagonal matrix `dinv`, x block = rin_I
     const double *stream = diag ? a.dinv : a.vals;
     const double *xsrc = diag ? a.rin : a.vin;
-    int64_t R0, R1;
+    int64_t R0, R1, P0, P1;   // owned rows [R0, R1), streamed blocks [P0, P1)
     if (ex.part != nullptr) {
-        R0 = ex.part[blockIdx.x];
-        R1 = ex.part[blockIdx.x + 1];
+        P0 = ex.part[2 * blockIdx.x];
+        R0 = ex.part[2 * blockIdx.x + 1];
+        P1 = ex.part[2 * blockIdx.x + 2];
+        R1 = ex.part[2 * blockIdx.x + 3];
     } else {
         R0 = a.n_brows * blockIdx.x / gridDim.x;
         R1 = a.n_brows * (blockIdx.x + 1) / gridDim.x;
+        P0 = R0;
+        P1 = R1;
     }
-    if (R0 >= R1) return;
-    const int64_t P0 = diag ? R0 : a.row_ptr[R0];
-    const int64_t P1 = diag ? R1 : a.row_ptr[R1];
+    if (P0 >= P1) return;
+    // head fragment: blocks [P0, row_ptr[R0]) belong to row R0-1, owned by the previous CTA
+    const bool head = !diag && (a.row_ptr[R0] > P0);
+    const int nitems = (int)(R1 - R0) + (head ? 1 : 0);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) {
@@ -209,26 +233,32 @@ __global__ void __launch_bounds__(TmaCfg::THREADS, 1) bsr_tma_kernel(const BsrAr
     if (spmv_scaled) inv_scale = 1.0 / *ex.scale_div;
 
     int seen = 0;  // last value read from `issued`
-    int64_t I = R0 + g;
+    // work items of this CTA: [the head fragment,] then the owned rows; group g takes items g, g+NG, ...
+    int it = g;
+    int64_t I = R0 + it - (head ? 1 : 0);
     int64_t p0 = 0, p1 = 0;
-    if (I < R1) {
+    if (it < nitems) {
         p0 = diag ? I : a.row_ptr[I];
         p1 = diag ? I + 1 : a.row_ptr[I + 1];
     }
-    for (; I < R1; I += C::NG) {
+    for (; it < nitems; it += C::NG, I += C::NG) {
         // next row's extent (off the critical path)
         const int64_t In = I + C::NG;
         int64_t p0n = 0, p1n = 0;
-        if (In < R1) {
+        if (it + C::NG < nitems) {
             p0n = diag ? In : a.row_ptr[In];
             p1n = diag ? In + 1 : a.row_ptr[In + 1];
         }
+        const bool frag = head && it == 0;     // the tail of row R0-1: partial sums go to the owner CTA
+        const bool open = p1 > P1;             // this row continues in the next CTA, which publishes its part
+        if (frag) p0 = P0;
+        if (open) p1 = P1;
         const size_t gi = (size_t)I * B + r;
         double rin_v = 0.0, dold = 0.0, xold = 0.0;
         double dreg[C::SEGL];
 #pragma unroll
         for (int c = 0; c < C::SEGL; ++c) dreg[c] = 0.0;
-        if (active) {
+        if (active && !frag) {
             if (a.mode == MODE_RESID || sweep) rin_v = a.rin[gi];
             if (sweep || (spmv_scaled && ex.vout != nullptr)) dold = a.vin[gi];
             if (touch_x && !(flags & F_SET_X)) xold = a.x[gi];
@@ -272,6 +302,32 @@ __global__ void __launch_bounds__(TmaCfg::THREADS, 1) bsr_tma_kernel(const BsrAr
         double acc = (acc0 + acc1) + acc2;
         acc += __shfl_xor_sync(0xffffffffu, acc, 1);
         acc += __shfl_xor_sync(0xffffffffu, acc, 2);
+
+        if (frag) {
+            // publish the 36 partial sums of the straddling row to its owner (CTA blockIdx.x - 1), then go on
+            if (writer) ex.frag_part[(size_t)blockIdx.x * B + r] = acc;
+            __threadfence();
+            group_bar(g);
+            if (t == 0) {
+                __threadfence();
+                atomicExch(ex.frag_flag + blockIdx.x, 1);
+            }
+            p0 = p0n;
+            p1 = p1n;
+            continue;
+        }
+        if (open) {
+            // the rest of this row was multiplied by CTA blockIdx.x + 1 as its FIRST work item: it is there by now
+            if (t == 0) {
+                while (atomicAdd(ex.frag_flag + blockIdx.x + 1, 0) == 0) {
+                }
+                __threadfence();
+            }
+            group_bar(g);
+            if (active) acc += __ldcg(ex.frag_part + (size_t)(blockIdx.x + 1) * B + r);
+            group_bar(g);
+            if (t == 0) atomicExch(ex.frag_flag + blockIdx.x + 1, 0);   // ready for the next launch
+        }
 
         if (a.mode == MODE_SPMV) {
             if (writer) {

@@ -77,6 +77,8 @@ struct mg_handle {
     int b = 0, n_pol = 0, n_phi = 0, n_levels = 0;
     int sm_count = 148;
     bool coop_ok = false;    // cooperative launches available and gmres_orth_fused_kernel's shared memory opted in
+    double *frag_part = nullptr;  // TMA kernel: partial sums of rows that straddle two CTAs (sm_count x 36)
+    int *frag_flag = nullptr;
     bool tma_ready = false;  // b == 36 and the kernel's shared-memory attribute is set
     cudaStream_t stream = nullptr;      // active stream: the caller's, or cap_stream while a graph is captured
     cudaStream_t cap_stream = nullptr;  // internal non-default stream (the legacy default stream cannot capture)
@@ -228,7 +230,7 @@ inline int grid_for(int64_t n, int per_block, int cap = 148 * 16) {
 }
 
 // ------------------------------------------------------------------------------------------------ BSR launch
-int launch_bsr(mg_handle *h, const Level &L, BsrArgs a, TmaExtra ex = TmaExtra{nullptr, nullptr, nullptr}) {
+int launch_bsr(mg_handle *h, const Level &L, BsrArgs a, TmaExtra ex = TmaExtra{}) {
     a.row_ptr = L.row_ptr;
     a.col_idx = L.col_idx;
     a.vals = L.vals;
@@ -241,6 +243,8 @@ int launch_bsr(mg_handle *h, const Level &L, BsrArgs a, TmaExtra ex = TmaExtra{n
     if (h->tma_ready && h->opt.kernel_variant == 0 && L.part != nullptr) {
         int grid = L.tma_grid;
         ex.part = L.part;
+        ex.frag_part = h->frag_part;
+        ex.frag_flag = h->frag_flag;
         if (a.mode == MODE_PBJ) {  // implicit block-diagonal stream: uniform split
             ex.part = nullptr;
             grid = (int)std::min<int64_t>(h->sm_count, L.n_brows);
@@ -562,7 +566,9 @@ int coarse_cycle_enqueue_fused(mg_handle *h) {
         a.vin = sj;
         a.out = sn;
         a.done = done;
-        TmaExtra ex{nullptr, G.dev.hnext, G.V + (size_t)j * G.stride};
+        TmaExtra ex{};
+        ex.scale_div = G.dev.hnext;
+        ex.vout = G.V + (size_t)j * G.stride;
         MG(launch_bsr(h, Lhat, a, ex));
         MG(gmres_orth(h, G, j, false, sn));
     }
@@ -819,9 +825,24 @@ void galerkin_symbolic(const Level &F, int n_pol, std::vector<int64_t> &crow_ptr
 int setup_level_partition(mg_handle *h, Level &L) {
     if (!h->tma_ready || L.n_brows == 0) return MG_OK;
     L.tma_grid = (int)std::min<int64_t>(h->sm_count, L.n_brows);
-    MG(dalloc_t(h, &L.part, (size_t)L.tma_grid + 1));
-    LAUNCH(h, partition_rows_kernel, (L.tma_grid + 1 + 127) / 128, 128, 0, L.row_ptr, L.n_brows, L.nnzb, L.tma_grid, L.part);
+    MG(dalloc_t(h, &L.part, 2 * ((size_t)L.tma_grid + 1)));
+    // equal block counts per CTA (a row may straddle two CTAs) when every CTA's range holds at least two whole rows;
+    // otherwise row-aligned ranges
+    int *d_max = nullptr;
+    MG(dalloc_t(h, &d_max, 4));
+    CU(cudaMemsetAsync(d_max, 0, sizeof(int), h->stream));
+    LAUNCH(h, max_row_blocks_kernel, grid_for(L.n_brows, 256, 1024), 256, 0, L.row_ptr, L.n_brows, d_max);
+    int hmax = 0;
+    CU(cudaMemcpyAsync(&hmax, d_max, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    const int split = (hmax > 0 && L.nnzb / L.tma_grid >= 3 * (int64_t)hmax) ? 1 : 0;
+    LAUNCH(h, partition_rows_kernel, (L.tma_grid + 1 + 127) / 128, 128, 0, L.row_ptr, L.n_brows, L.nnzb, L.tma_grid, split, L.part);
     CU(cudaGetLastError());
+    if (h->frag_part == nullptr) {
+        MG(dalloc_t(h, &h->frag_part, (size_t)h->sm_count * TmaCfg::B));
+        MG(dalloc_t(h, &h->frag_flag, (size_t)h->sm_count));
+        CU(cudaMemsetAsync(h->frag_flag, 0, sizeof(int) * h->sm_count, h->stream));
+    }
     return MG_OK;
 }
 
