@@ -17,6 +17,8 @@ CASES = {
     "b12-3lev": dict(name="C0", mesh=(5, 16), n_phi=8, levels=3, b=12, seed=77),
     "b6-4lev": dict(name="C0", mesh=(6, 20), n_phi=16, levels=4, b=6, seed=78),
     "b5-generic-to-1-plane": dict(name="C0", mesh=(3, 8), n_phi=4, levels=3, b=5, seed=79),
+    # b = 36 at small size: the TMA-ring kernel, GMRES on the precomputed A D^-1 and the fused CGS2 (the bench path)
+    "b36-3lev": dict(name="C0", mesh=(3, 10), n_phi=8, levels=3, seed=85),
 }
 
 
@@ -42,7 +44,7 @@ def test_vcycle_pinned_coarse_mode(case, nu):
         s.destroy()
 
 
-@pytest.mark.parametrize("case", ["b12-3lev", "b6-4lev", "b5-generic-to-1-plane"])
+@pytest.mark.parametrize("case", ["b12-3lev", "b6-4lev", "b5-generic-to-1-plane", "b36-3lev"])
 def test_vcycle_default_mode_residual_sense(case):
     """PBJ-GMRES coarse solve on both sides, coarse_rtol tightened to 1e-13: the cycles agree in the residual
     sense ||A (z_gpu - z_or)||_inf / ||r||_inf <= 1e-8 (the coarse corrections agree only to cond * rtol)."""
@@ -57,7 +59,7 @@ def test_vcycle_default_mode_residual_sense(case):
         s.destroy()
 
 
-@pytest.mark.parametrize("case", ["b12-3lev", "b6-4lev", "b5-generic-to-1-plane"])
+@pytest.mark.parametrize("case", ["b12-3lev", "b6-4lev", "b5-generic-to-1-plane", "b36-3lev"])
 @pytest.mark.parametrize("graphs", [1, 0])
 def test_coarse_solve(case, graphs):
     """PBJ-GMRES(100) to 1e-10 on the coarsest level: both reach the tolerance; the solutions agree to
