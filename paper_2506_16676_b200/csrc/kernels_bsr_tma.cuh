@@ -41,6 +41,8 @@ struct TmaCfg {
     static constexpr int STAGES = 20;
     static constexpr int THREADS = NG * GROUP + 32;   // + 1 producer warp
     static constexpr int VECPAD = 40;
+    static constexpr unsigned POLL_NS = 1000;         // sleep between polls of the producer's `issued` counter
+    static constexpr unsigned SWEEP_MBAR_NS = 100;    // back-off of the full-barrier wait in the fused sweep
     static constexpr size_t SMEM = sizeof(double) * ((size_t)STAGES * (BB + B) + NG * VECPAD) + sizeof(uint64_t) * (2 * STAGES + 2);
 };
 
@@ -81,6 +83,24 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
             : "memory");
     } while (!ok);
 }
+// Same, with a back-off between polls (ns = 0: none).  Waiting consumer warps otherwise compete with the producer warp
+// and with the group that is in its row epilogue for issue slots (measured: see DESIGN.md 5.1).
+__device__ __forceinline__ void mbar_wait_backoff(uint64_t *bar, uint32_t parity, unsigned ns) {
+    uint32_t ok;
+    while (true) {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n"
+            : "=r"(ok)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+        if (ok) break;
+        if (ns) __nanosleep(ns);
+    }
+}
 // 1-D bulk async copy global -> shared, completing `bytes` on the mbarrier (TMA engine; SASS UBLKCP).
 __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
@@ -103,8 +123,6 @@ __device__ __forceinline__ void group_bar(int g) {
     asm volatile("bar.sync %0, %1;" ::"r"(g + 1), "n"(TmaCfg::GROUP) : "memory");
 }
 
-// part[k] = first block row I with row_ptr[I] >= k * nnzb / nparts (k = 0..nparts; part[nparts] = n_brows):
-// contiguous row ranges holding (nearly) equal numbers of blocks.
 // max over block rows of the number of stored blocks
 __global__ void max_row_blocks_kernel(const int64_t *__restrict__ row_ptr, const int64_t n_brows, int *__restrict__ out) {
     int m = 0;
@@ -232,6 +250,7 @@ __global__ void __launch_bounds__(TmaCfg::THREADS, 1) bsr_tma_kernel(const BsrAr
     const bool spmv_scaled = (a.mode == MODE_SPMV) && ex.scale_div != nullptr;
     if (spmv_scaled) inv_scale = 1.0 / *ex.scale_div;
 
+    const unsigned mbar_ns = need_d ? C::SWEEP_MBAR_NS : 0u;   // back off only when row epilogues are heavy
     int seen = 0;  // last value read from `issued`
     // work items of this CTA: [the head fragment,] then the owned rows; group g takes items g, g+NG, ...
     int it = g;
@@ -274,11 +293,13 @@ __global__ void __launch_bounds__(TmaCfg::THREADS, 1) bsr_tma_kernel(const BsrAr
         double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0;
         for (int64_t p = p0; p < p1; ++p, ++n) {
             if (n >= seen) {
-                do {
+                seen = *issued;
+                while (n >= seen) {   // not issued yet: sleep instead of spinning on shared memory (5-6 % on every level)
+                    __nanosleep(C::POLL_NS);
                     seen = *issued;
-                } while (n >= seen);
+                }
             }
-            mbar_wait(&full[s], ph);
+            mbar_wait_backoff(&full[s], ph, mbar_ns);
             if (active) {
                 const double *A = sA + (size_t)s * BB + C::SEGL * t;
                 const double *xs = sX + s * B + C::SEGL * h;
