@@ -37,13 +37,13 @@ struct TmaCfg {
     static constexpr int ACTIVE = B * SEG;            // 144 working threads per group
     static constexpr int GROUP = 160;                 // 5 warps per group (16 idle lanes)
     static constexpr int GWARPS = GROUP / 32;
-    static constexpr int NG = 4;                      // consumer groups per CTA
+    static constexpr int NG = 4;                      // consumer groups per CTA (3: -8 %, 5: no gain)
     static constexpr int STAGES = 20;
     static constexpr int THREADS = NG * GROUP + 32;   // + 1 producer warp
     static constexpr int VECPAD = 40;
-    static constexpr unsigned POLL_NS = 1000;         // sleep between polls of the producer's `issued` counter
+    static constexpr unsigned POLL_NS = 1000;         // sleep between polls of the producer's per-stage round counters
     static constexpr unsigned SWEEP_MBAR_NS = 100;    // back-off of the full-barrier wait in the fused sweep
-    static constexpr size_t SMEM = sizeof(double) * ((size_t)STAGES * (BB + B) + NG * VECPAD) + sizeof(uint64_t) * (2 * STAGES + 2);
+    static constexpr size_t SMEM = sizeof(double) * ((size_t)STAGES * (BB + B) + NG * VECPAD) + sizeof(uint64_t) * (3 * STAGES);
 };
 
 // extra arguments of the TMA kernel (the common ones are BsrArgs)
@@ -164,11 +164,11 @@ __global__ void __launch_bounds__(TmaCfg::THREADS, 1) bsr_tma_kernel(const BsrAr
     double *sVec = sX + C::STAGES * B;
     uint64_t *full = reinterpret_cast<uint64_t *>(sVec + C::NG * C::VECPAD);
     uint64_t *empty = full + C::STAGES;
-    // number of blocks the producer has issued so far.  A consumer group may be more than one ring round ahead of
-    // the stage it wants next (its row starts >= STAGES blocks after the oldest block still in flight); an
-    // mbarrier parity wait is only meaningful for the current or the preceding phase, so the group first waits
+    // round_of[s] = number of rounds for which stage s has been issued.  A consumer group may be more than one ring
+    // round ahead of the stage it wants next (its row starts >= STAGES blocks after the oldest block still in flight);
+    // an mbarrier parity wait is only meaningful for the current or the preceding phase, so the group first waits
     // until its block has been ISSUED (then the stage's previous round is consumed and its phase is the current one).
-    volatile int *issued = reinterpret_cast<volatile int *>(empty + C::STAGES);
+    volatile int *round_of = reinterpret_cast<volatile int *>(empty + C::STAGES);   // [STAGES]
 
     const bool diag = (a.mode == MODE_PBJ);             // implicit block-diagonal matrix `dinv`, x block = rin_I
     const double *stream = diag ? a.dinv : a.vals;
@@ -192,7 +192,7 @@ __global__ void __launch_bounds__(TmaCfg::THREADS, 1) bsr_tma_kernel(const BsrAr
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) {
-        *issued = 0;
+        for (int s = 0; s < C::STAGES; ++s) round_of[s] = 0;
         for (int s = 0; s < C::STAGES; ++s) {
             mbar_init(&full[s], 1);
             mbar_init(&empty[s], C::GWARPS);
@@ -205,33 +205,25 @@ __global__ void __launch_bounds__(TmaCfg::THREADS, 1) bsr_tma_kernel(const BsrAr
         // ------------------------------------------------------------------ producer warp: stream blocks P0..P1
         const uint64_t pol = policy_evict_first();
         const int total = (int)(P1 - P0);
-        int cnext = 0;
-        if (lane < total) cnext = diag ? (int)(P0 + lane) : __ldg(a.col_idx + P0 + lane);
-        int s = 0;
-        uint32_t ph = 0;
-        for (int base = 0; base < total; base += 32) {
-            const int c = cnext;
-            const int nb = base + 32 + lane;
-            if (nb < total) cnext = diag ? (int)(P0 + nb) : __ldg(a.col_idx + P0 + nb);
-            const int cnt = min(32, total - base);
-            for (int i = 0; i < cnt; ++i) {
-                const int j = __shfl_sync(0xffffffffu, c, i);
-                if (lane == 0) {
-                    mbar_wait(&empty[s], ph ^ 1u);
-                    mbar_expect_tx(&full[s], (uint32_t)((BB + B) * sizeof(double)));
-                    // the matrix stream is read once per launch: evict-first keeps the vectors, the Krylov basis and (on
-                    // small levels) Dinv resident in the 126 MB L2; Dinv itself (PBJ apply) is loaded with the default policy
-                    if (diag) bulk_g2s(sA + (size_t)s * BB, stream + (size_t)(P0 + base + i) * BB, BB * sizeof(double), &full[s]);
-                    else bulk_g2s_hint(sA + (size_t)s * BB, stream + (size_t)(P0 + base + i) * BB, BB * sizeof(double), &full[s], pol);
-                    bulk_g2s(sX + s * B, xsrc + (size_t)j * B, B * sizeof(double), &full[s]);
-                    __threadfence_block();
-                    *issued = base + i + 1;
-                }
-                if (++s == C::STAGES) {
-                    s = 0;
-                    ph ^= 1u;
-                }
+        // Every lane < PL issues its own block: the waits on the stages' "empty" barriers and the issue latencies
+        // overlap (one issuing thread was the pacing element of the whole kernel: +5-7 % on levels 1-3).  round_of[s]
+        // tells the consumers that stage s has been (re)issued for round k, see above.
+        constexpr int PL = 16;
+        for (int base = 0; base < total; base += PL) {
+            const int i = base + lane;
+            if (lane < PL && i < total) {
+                const int j = diag ? (int)(P0 + i) : __ldg(a.col_idx + P0 + i);
+                const int s = i % C::STAGES, k = i / C::STAGES;
+                mbar_wait(&empty[s], ((uint32_t)k & 1u) ^ 1u);
+                round_of[s] = k + 1;
+                mbar_expect_tx(&full[s], (uint32_t)((BB + B) * sizeof(double)));
+                // the matrix stream is read once per launch: evict-first keeps the vectors, the Krylov basis and (on small
+                // levels) Dinv resident in the 126 MB L2; Dinv itself (PBJ apply) is loaded with the default policy
+                if (diag) bulk_g2s(sA + (size_t)s * BB, stream + (size_t)(P0 + i) * BB, BB * sizeof(double), &full[s]);
+                else bulk_g2s_hint(sA + (size_t)s * BB, stream + (size_t)(P0 + i) * BB, BB * sizeof(double), &full[s], pol);
+                bulk_g2s(sX + s * B, xsrc + (size_t)j * B, B * sizeof(double), &full[s]);
             }
+            __syncwarp();
         }
         return;
     }
@@ -251,7 +243,6 @@ __global__ void __launch_bounds__(TmaCfg::THREADS, 1) bsr_tma_kernel(const BsrAr
     if (spmv_scaled) inv_scale = 1.0 / *ex.scale_div;
 
     const unsigned mbar_ns = need_d ? C::SWEEP_MBAR_NS : 0u;   // back off only when row epilogues are heavy
-    int seen = 0;  // last value read from `issued`
     // work items of this CTA: [the head fragment,] then the owned rows; group g takes items g, g+NG, ...
     int it = g;
     int64_t I = R0 + it - (head ? 1 : 0);
@@ -292,13 +283,8 @@ __global__ void __launch_bounds__(TmaCfg::THREADS, 1) bsr_tma_kernel(const BsrAr
         uint32_t ph = (uint32_t)(n / C::STAGES) & 1u;
         double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0;
         for (int64_t p = p0; p < p1; ++p, ++n) {
-            if (n >= seen) {
-                seen = *issued;
-                while (n >= seen) {   // not issued yet: sleep instead of spinning on shared memory (5-6 % on every level)
-                    __nanosleep(C::POLL_NS);
-                    seen = *issued;
-                }
-            }
+            // not (re)issued for this round yet: sleep instead of spinning on shared memory (5-6 % on every level)
+            while (round_of[s] <= n / C::STAGES) __nanosleep(C::POLL_NS);
             mbar_wait_backoff(&full[s], ph, mbar_ns);
             if (active) {
                 const double *A = sA + (size_t)s * BB + C::SEGL * t;
