@@ -76,6 +76,10 @@ typedef struct mg_options {
     int smoother;            /* 0 (default): PBJ-Chebyshev (BASELINE.json north_star); 1: nu iterations of right-PBJ-
                                 preconditioned GMRES without a convergence test -- the paper's own level smoother,
                                 "one iteration of GMRES preconditioned with PBJ", V(1,1) / V(6,6) */
+    double orth_eta;         /* Gram-Schmidt in (F)GMRES: 0 = classical Gram-Schmidt with a second pass on every step
+                                (CGS2); eta in (0,1) = the second pass only when ||w - V V^T w|| < eta ||w|| (selective
+                                reorthogonalisation, Daniel-Gragg-Kaufman-Stewart).  Same Arnoldi relation either way.
+                                Default 0.25 (orthogonality kept to ~4 eps per step). */
     mg_alloc_fn alloc;       /* NULL => cudaMalloc */
     mg_free_fn free;         /* NULL => cudaFree */
     void *alloc_ctx;

@@ -248,6 +248,8 @@ struct OrthArgs {
     int slice;             // elements per CTA, even
     int cap;               // basis vectors cached in shared memory
     int ld;                // >= m + 1
+    double eta2;           // selective reorthogonalisation (Daniel-Gragg-Kaufman-Stewart): the second pass is skipped
+                           // when ||w - V h1||^2 >= eta2 ||w||^2, estimated as ||w||^2 - |h1|^2; 0 = always two passes
 };
 #ifndef MG_ORTH_STAMP   // development probe: per-phase clock stamps (compiled out in the library)
 #define MG_ORTH_STAMP(k)
@@ -331,34 +333,58 @@ __global__ void __launch_bounds__(ORTH_THREADS, 1) gmres_orth_fused_kernel(const
             s = warp_sum(s);
             if (lane == 0) hd[item] = s;
         }
+        // pass 0 also reduces <w, w> (entry nvec): it decides whether a second pass is needed
+        const int nred = nvec + ((pass == 0 && a.eta2 > 0.0) ? 1 : 0);
+        if (nred > nvec) {
+            double sq = 0.0;
+            for (int e = tid; e < len; e += ORTH_THREADS) sq = fma(ws[e], ws[e], sq);
+            sq = warp_sum(sq);
+            if (lane == 0) red[warp] = sq;
+        }
         __syncthreads();
         for (int i = tid; i < nvec; i += ORTH_THREADS) a.partial[(size_t)blockIdx.x * a.ld + i] = hd[2 * i] + hd[2 * i + 1];
+        if (nred > nvec && tid == 0) {
+            double t = 0.0;
+            for (int k = 0; k < NW; ++k) t += red[k];
+            a.partial[(size_t)blockIdx.x * a.ld + nvec] = t;
+        }
         MG_ORTH_STAMP(2 + 4 * pass);
         grid.sync();
         MG_ORTH_STAMP(3 + 4 * pass);
         // ---- h_i = sum over CTAs: 8 interleaved sub-ranges in parallel (19 independent loads each), fixed order
         double *hout = (pass == 0) ? a.dev.h1 : a.dev.h2;
-        for (int i0 = 0; i0 < nvec; i0 += 64) {
+        for (int i0 = 0; i0 < nred; i0 += 64) {
             const int il = tid & 63, q = tid >> 6, i = i0 + il;
             double pv[ORTH_MAX_GRID / 8];
 #pragma unroll
             for (int u = 0; u < ORTH_MAX_GRID / 8; ++u) {
                 const int c = q + 8 * u;
-                pv[u] = (i < nvec && c < G) ? __ldcg(a.partial + (size_t)c * a.ld + i) : 0.0;
+                pv[u] = (i < nred && c < G) ? __ldcg(a.partial + (size_t)c * a.ld + i) : 0.0;
             }
             double s = 0.0;
 #pragma unroll
             for (int u = 0; u < ORTH_MAX_GRID / 8; ++u) s += pv[u];
             red[q * 64 + il] = s;
             __syncthreads();
-            if (q == 0 && i < nvec) {
+            if (q == 0 && i < nred) {
                 double t = 0.0;
 #pragma unroll
                 for (int qq = 0; qq < 8; ++qq) t += red[qq * 64 + il];
                 hs[i] = t;
-                if (blockIdx.x == 0) hout[i] = t;
+                if (blockIdx.x == 0 && i < nvec) hout[i] = t;
             }
             __syncthreads();
+        }
+        // every CTA sums the same partials in the same order, so every CTA takes the same decision
+        bool skip_second = false;
+        if (nred > nvec) {
+            if (tid == 0) {
+                double s2 = 0.0;
+                for (int i = 0; i < nvec; ++i) s2 = fma(hs[i], hs[i], s2);
+                red[0] = (hs[nvec] - s2 >= a.eta2 * hs[nvec]) ? 1.0 : 0.0;
+            }
+            __syncthreads();
+            skip_second = red[0] != 0.0;
         }
         MG_ORTH_STAMP(4 + 4 * pass);
         // ---- w_slice -= sum_i h_i V_i : one double2 per thread, two independent accumulator pairs
@@ -397,6 +423,11 @@ __global__ void __launch_bounds__(ORTH_THREADS, 1) gmres_orth_fused_kernel(const
         }
         __syncthreads();
         MG_ORTH_STAMP(5 + 4 * pass);
+        if (skip_second) {
+            if (blockIdx.x == 0)
+                for (int i = tid; i < nvec; i += ORTH_THREADS) a.dev.h2[i] = 0.0;
+            break;
+        }
     }
     // ---- write back, ||w||^2, Hessenberg column / Givens / stop test in the last CTA
     double sq = 0.0;

@@ -502,6 +502,7 @@ int gmres_orth(mg_handle *h, Gmres &G, int j, bool normalize = true, double *w_o
         oa.slice = G.orth_slice;
         oa.cap = G.orth_cap;
         oa.ld = G.orth_ld;
+        oa.eta2 = h->opt.orth_eta * h->opt.orth_eta;
         void *params[] = {&oa};
         ProfPair pp;
         const bool prof = prof_begin(h, pp);
@@ -966,6 +967,7 @@ int mg_options_default(mg_options *o) {
     o->use_graphs = 1;
     o->kernel_variant = 0;
     o->smoother = 0;
+    o->orth_eta = 0.25;
     return MG_OK;
 }
 
@@ -977,6 +979,7 @@ static int validate_options(const mg_options &o) {
     if (o.restart < 1 || o.maxit < 1 || o.block_layout != 0) return MG_EINVAL;
     if (o.kernel_variant < 0 || o.kernel_variant > 1) return MG_EINVAL;
     if (o.smoother < 0 || o.smoother > 1) return MG_EINVAL;
+    if (!(o.orth_eta >= 0.0) || o.orth_eta >= 1.0) return MG_EINVAL;
     return MG_OK;
 }
 
@@ -1095,7 +1098,7 @@ int mg_update_options(mg_handle *h, const mg_options *opt) {
     o.block_layout = h->opt.block_layout;
     if (validate_options(o) != MG_OK) return MG_EINVAL;
     const bool bounds = (o.cheb_lo != h->opt.cheb_lo) || (o.cheb_hi != h->opt.cheb_hi);
-    if (o.kernel_variant != h->opt.kernel_variant && h->coarse_graph) {  // the captured cycle holds the old kernels
+    if ((o.kernel_variant != h->opt.kernel_variant || o.orth_eta != h->opt.orth_eta) && h->coarse_graph) {  // the captured cycle holds the old kernels
         cudaStreamSynchronize(h->stream);
         cudaGraphExecDestroy(h->coarse_graph);
         h->coarse_graph = nullptr;

@@ -24,7 +24,7 @@ def small(name="C0", **kw):
     return make_workload(name, **kw)
 
 
-GPU_ONLY_OPTIONS = ("use_graphs", "kernel_variant")   # launch mechanics of the CUDA library; no arithmetic meaning
+GPU_ONLY_OPTIONS = ("use_graphs", "kernel_variant", "orth_eta")   # launch mechanics of the CUDA library; no arithmetic meaning
 
 
 def oracle_hierarchy(w, **opt):
