@@ -97,6 +97,9 @@ typedef struct mg_solve_info {
 
 /* Fill *opt with the defaults above.  Returns MG_EINVAL if opt is NULL. */
 int mg_options_default(mg_options *opt);
+/* sizeof(mg_options) / sizeof(mg_solve_info) as this library was compiled: a binding checks its own layout against them. */
+size_t mg_sizeof_options(void);
+size_t mg_sizeof_solve_info(void);
 
 /* mg_setup -- build the hierarchy ("the batched diagonal-block inversion and ... the Galerkin coarse
  * operators", north_star).  Per level: locate and invert every diagonal block

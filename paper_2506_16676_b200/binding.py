@@ -36,6 +36,8 @@ class mg_solve_info(C.Structure):
 _VP, _I, _D, _I64 = C.c_void_p, C.c_int, C.c_double, C.c_int64
 SYMBOLS = {
     "mg_options_default": (_I, [C.POINTER(mg_options)]),
+    "mg_sizeof_options": (C.c_size_t, []),
+    "mg_sizeof_solve_info": (C.c_size_t, []),
     "mg_setup": (_I, [C.POINTER(_VP), _VP, _VP, _VP, _I, _I, _I, _I, C.POINTER(mg_options), _VP]),
     "mg_update_options": (_I, [_VP, C.POINTER(mg_options)]),
     "mg_update_values": (_I, [_VP, _VP]),
@@ -84,6 +86,9 @@ def lib():
         for name, (res, args) in SYMBOLS.items():
             fn = getattr(L, name)
             fn.restype, fn.argtypes = res, args
+        if L.mg_sizeof_options() != C.sizeof(mg_options) or L.mg_sizeof_solve_info() != C.sizeof(mg_solve_info):
+            raise RuntimeError("binding.py and libmgtoroidal.so disagree on the layout of mg_options / mg_solve_info: "
+                               "rebuild with paper_2506_16676_b200.buildlib.build(force=True)")
         _lib = L
     return _lib
 

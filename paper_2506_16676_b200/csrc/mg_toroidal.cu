@@ -971,6 +971,9 @@ int mg_options_default(mg_options *o) {
     return MG_OK;
 }
 
+size_t mg_sizeof_options(void) { return sizeof(mg_options); }
+size_t mg_sizeof_solve_info(void) { return sizeof(mg_solve_info); }
+
 static int validate_options(const mg_options &o) {
     if (o.nu_pre < 0 || o.nu_post < 0 || o.eig_iters < 1) return MG_EINVAL;
     if (!(o.cheb_lo > 0.0) || !(o.cheb_hi > o.cheb_lo)) return MG_EINVAL;

@@ -48,6 +48,15 @@ def test_options_default_values():
     assert binding.lib().mg_options_default(None) == binding.MG_EINVAL
 
 
+def test_binding_struct_layouts_match_the_library(lib):
+    lib.mg_sizeof_options.restype = ctypes.c_size_t
+    lib.mg_sizeof_solve_info.restype = ctypes.c_size_t
+    assert lib.mg_sizeof_options() == ctypes.sizeof(binding.mg_options)
+    assert lib.mg_sizeof_solve_info() == ctypes.sizeof(binding.mg_solve_info)
+    o = binding.options_default()
+    assert (o.smoother, o.kernel_variant, o.use_graphs) == (0, 0, 1) and o.orth_eta == 0.25   # last fields land where C put them
+
+
 def test_strerror_and_version():
     assert binding.strerror(0) == "ok"
     assert "singular" in binding.strerror(binding.MG_ESINGULAR)
