@@ -240,7 +240,8 @@ struct OrthArgs {
     int j;                 // orthogonalise against V_0..V_j
     double *w;             // V_{j+1}, updated in place
     int64_t n;
-    double *partial;       // [gridDim.x][ld]
+    double *partial;       // [ORTH_REPLICAS][gridDim.x][ld]: every CTA reads all partials after the barrier; replicas at
+                           // different addresses spread that hot spot over more L2 slices (CTA c reads replica c % R)
     double *nrm_partial;   // [gridDim.x]
     unsigned *counter;     // ticket of the final norm, zero-initialised, self-resetting
     GmresDev dev;
@@ -255,6 +256,7 @@ struct OrthArgs {
 #define MG_ORTH_STAMP(k)
 #endif
 constexpr int ORTH_THREADS = 512;
+constexpr int ORTH_REPLICAS = 8;
 constexpr int ORTH_MAX_GRID = 152;          // 8 * 19: the cross-CTA reduction unrolls over 19 loads per thread
 constexpr int ORTH_SCRATCH = 8 * 64 + 32;   // doubles of reduction scratch (+ 2*ld for the half-slice dots)
 inline size_t orth_smem_bytes(int slice, int ld, int cap) {
@@ -342,11 +344,17 @@ __global__ void __launch_bounds__(ORTH_THREADS, 1) gmres_orth_fused_kernel(const
             if (lane == 0) red[warp] = sq;
         }
         __syncthreads();
-        for (int i = tid; i < nvec; i += ORTH_THREADS) a.partial[(size_t)blockIdx.x * a.ld + i] = hd[2 * i] + hd[2 * i + 1];
+        const size_t rep_stride = (size_t)G * a.ld;
         if (nred > nvec && tid == 0) {
             double t = 0.0;
             for (int k = 0; k < NW; ++k) t += red[k];
-            a.partial[(size_t)blockIdx.x * a.ld + nvec] = t;
+            hd[2 * nvec] = t;
+            hd[2 * nvec + 1] = 0.0;
+        }
+        __syncthreads();
+        for (int i = tid; i < nred * ORTH_REPLICAS; i += ORTH_THREADS) {
+            const int rep = i / nred, ii = i - rep * nred;
+            a.partial[rep * rep_stride + (size_t)blockIdx.x * a.ld + ii] = hd[2 * ii] + hd[2 * ii + 1];
         }
         MG_ORTH_STAMP(2 + 4 * pass);
         grid.sync();
@@ -359,7 +367,7 @@ __global__ void __launch_bounds__(ORTH_THREADS, 1) gmres_orth_fused_kernel(const
 #pragma unroll
             for (int u = 0; u < ORTH_MAX_GRID / 8; ++u) {
                 const int c = q + 8 * u;
-                pv[u] = (i < nred && c < G) ? __ldcg(a.partial + (size_t)c * a.ld + i) : 0.0;
+                pv[u] = (i < nred && c < G) ? __ldcg(a.partial + (blockIdx.x % ORTH_REPLICAS) * rep_stride + (size_t)c * a.ld + i) : 0.0;
             }
             double s = 0.0;
 #pragma unroll

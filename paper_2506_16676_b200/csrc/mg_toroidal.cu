@@ -450,7 +450,7 @@ int gmres_alloc(mg_handle *h, Gmres &G, int64_t n, int m, int maxit, bool flexib
             const size_t left = budget - orth_smem_bytes(G.orth_slice, G.orth_ld, 0);
             G.orth_cap = (int)std::min<size_t>(left / (sizeof(double) * G.orth_slice), (size_t)m + 1);
             G.orth_smem = orth_smem_bytes(G.orth_slice, G.orth_ld, G.orth_cap);
-            MG(dalloc_t(h, &G.orth_partial, (size_t)G.orth_grid * G.orth_ld));
+            MG(dalloc_t(h, &G.orth_partial, (size_t)ORTH_REPLICAS * G.orth_grid * G.orth_ld));
             MG(dalloc_t(h, &G.orth_nrm, (size_t)G.orth_grid));
             MG(dalloc_t(h, &G.orth_counter, 2));
             CU(cudaMemsetAsync(G.orth_counter, 0, 2 * sizeof(unsigned), h->stream));
