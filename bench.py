@@ -162,7 +162,7 @@ def oracle_sample(w, seconds: float = 15.0):
         y = oracle_mg.spmv(L, x)
         oracle_mg.pbj_apply(L, y)
         reps += 1
-        if time.perf_counter() - t0 >= seconds or reps >= 200:
+        if time.perf_counter() - t0 >= seconds or reps >= 5000:
             break
     dt = time.perf_counter() - t0
     gbs = reps * (size.spmv() + size.pbj()) / dt / 1e9
