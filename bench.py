@@ -248,10 +248,10 @@ def cuda_arm(args):
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(replicas.env_world()[1])     # before the process group: NCCL binds to the current device
     rank, local_rank, world = replicas.init("nccl")
     if world != args.gpus:
         log(f"note: --gpus {args.gpus} but WORLD_SIZE {world}; using WORLD_SIZE")
-    torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     buildlib.build()
 
