@@ -445,7 +445,7 @@ def main():
     ap.add_argument("--steps", type=int, default=1)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
-    ap.add_argument("--workload", default="C1", help="C1 (the metric's config, default); C0, C2-16/32/64, C3 for other configs")
+    ap.add_argument("--workload", default="C1", help="C1 (the metric's config, default); C0, C2-16/32/64, C3, C3b for other configs")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="CPU time of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--max-outer", type=int, default=0,

@@ -75,6 +75,10 @@ CONFIGS = {
     "C2-64": dict(mesh=(20, 100), n_phi=64, levels=6, sigma=1e-4, beta=1.0, delta=0.05, b=36, seed=BASE_SEED + 2),
     "C3": dict(mesh=(40, 200), n_phi=32, levels=5, sigma=1e-4, beta=0.5, delta=0.15, b=36, seed=BASE_SEED + 3,
                nonaxisymmetric=True),
+    # C3b (Q16): config 3 with the 21-block prism stencil on the FINE level -- the density of
+    # the paper's matrices (~750 nnz/row) and the "~55 GB" that configs[3] states (54.9 GB).
+    "C3b": dict(mesh=(40, 200), n_phi=32, levels=5, sigma=1e-4, beta=0.5, delta=0.15, b=36, seed=BASE_SEED + 3,
+                nonaxisymmetric=True, prism=True),
 }
 
 
@@ -131,15 +135,16 @@ def poloidal_mesh(n_r: int, n_theta: int, rng: np.random.Generator):
 
 def make_workload(name: str = "C0", *, mesh=None, n_phi=None, levels=None, sigma=None, beta=None, delta=None,
                   b=None, seed=None, nonaxisymmetric=None, shuffle: bool = False, noise_chunk: int = 4096,
-                  want_rhs: bool = True) -> Workload:
+                  want_rhs: bool = True, prism=None) -> Workload:
     """Build one workload.  ``name`` selects a row of CONFIGS; keyword arguments override single fields
     (used by the tests for reduced-size variants of the same recipe)."""
     cfg = dict(CONFIGS[name]) if name in CONFIGS else {}
     for k, v in dict(mesh=mesh, n_phi=n_phi, levels=levels, sigma=sigma, beta=beta, delta=delta, b=b, seed=seed,
-                     nonaxisymmetric=nonaxisymmetric).items():
+                     nonaxisymmetric=nonaxisymmetric, prism=prism).items():
         if v is not None:
             cfg[k] = v
     cfg.setdefault("nonaxisymmetric", False)
+    cfg.setdefault("prism", False)
     n_r, n_theta = cfg["mesh"]
     n_phi_, b_ = int(cfg["n_phi"]), int(cfg["b"])
     sigma_, beta_, delta_ = float(cfg["sigma"]), float(cfg["beta"]), float(cfg["delta"])
@@ -176,7 +181,10 @@ def make_workload(name: str = "C0", *, mesh=None, n_phi=None, levels=None, sigma
     # ---- pattern: COO of all blocks, then sort by (row, col) -------------------------------------------------
     E = edges.shape[0]
     i_all = np.arange(n_pol, dtype=np.int64)
-    rows, cols, kind, ref = [], [], [], []
+    rows, cols, kind, ref, dpl = [], [], [], [], []   # dpl: plane offset of the column (-1, 0, +1)
+    prism_ = bool(cfg["prism"])
+    if prism_ and n_phi_ < 3:
+        raise ValueError("the prism stencil needs n_phi >= 3")
     for k in range(n_phi_):
         base = k * n_pol
         rows += [base + i_all, base + edges[:, 0], base + edges[:, 1], base + i_all, base + i_all]
@@ -185,12 +193,23 @@ def make_workload(name: str = "C0", *, mesh=None, n_phi=None, levels=None, sigma
         kind += [np.full(n_pol, 0, np.int8), np.full(E, 1, np.int8), np.full(E, 1, np.int8),
                  np.full(n_pol, 2, np.int8), np.full(n_pol, 2, np.int8)]
         ref += [i_all, np.arange(E, dtype=np.int64), np.arange(E, dtype=np.int64), i_all, i_all]
+        dpl += [np.zeros(n_pol, np.int8), np.zeros(E, np.int8), np.zeros(E, np.int8),
+                np.full(n_pol, -1, np.int8), np.full(n_pol, 1, np.int8)]
+        if prism_:  # edge blocks to the neighbouring planes: (i,k)-(j,k+-1)
+            for dk in (-1, 1):
+                nb = ((k + dk) % n_phi_) * n_pol
+                rows += [base + edges[:, 0], base + edges[:, 1]]
+                cols += [nb + edges[:, 1], nb + edges[:, 0]]
+                kind += [np.full(E, 3, np.int8), np.full(E, 3, np.int8)]
+                ref += [np.arange(E, dtype=np.int64), np.arange(E, dtype=np.int64)]
+                dpl += [np.full(E, dk, np.int8), np.full(E, dk, np.int8)]
     rows = np.concatenate(rows)
     cols = np.concatenate(cols)
     kind = np.concatenate(kind)
     ref = np.concatenate(ref)
+    dpl = np.concatenate(dpl)
     order = np.lexsort((cols, rows))
-    rows, cols, kind, ref = rows[order], cols[order], kind[order], ref[order]
+    rows, cols, kind, ref, dpl = rows[order], cols[order], kind[order], ref[order], dpl[order]
     nnzb = rows.shape[0]
     row_ptr = np.zeros(n + 1, dtype=np.int64)
     np.add.at(row_ptr, rows + 1, 1)
@@ -201,13 +220,42 @@ def make_workload(name: str = "C0", *, mesh=None, n_phi=None, levels=None, sigma
     # ---- deterministic part of the values ---------------------------------------------------------------------
     vals = np.empty((nnzb, b_, b_), dtype=np.float64)
     eye = np.eye(b_)
-    for k in range(n_phi_):
-        Sk = S if lam_k is None else (QS * lam_k[k][None, :]) @ QS.T
-        if lam_k is not None:
-            Sk = 0.5 * (Sk + Sk.T)
-        wsum = np.zeros(n_pol)
-        np.add.at(wsum, edges[:, 0], w_k[k])
-        np.add.at(wsum, edges[:, 1], w_k[k])
+    def S_of(k):
+        if lam_k is None:
+            return S
+        Sk_ = (QS * lam_k[k][None, :]) @ QS.T
+        return 0.5 * (Sk_ + Sk_.T)
+
+    def wsum_of(k):
+        ws_ = np.zeros(n_pol)
+        np.add.at(ws_, edges[:, 0], w_k[k])
+        np.add.at(ws_, edges[:, 1], w_k[k])
+        return ws_
+
+    if prism_:
+        # A = sigma I + sum over toroidal intervals (k, k+1) of W_{k+1/2} (x) [[1/3, 1/6], [1/6, 1/3]] + beta circ(-1,2,-1) (x) I (x) T,
+        # W_k = L_w^(k) (x) S^(k), W_{k+1/2} = (W_k + W_{k+1}) / 2: a sum of positive semi-definite Kronecker products (linear
+        # finite-element mass coupling along the torus).  Axisymmetric case: (L_w (x) S) (x) circ(1/6, 2/3, 1/6).
+        for k in range(n_phi_):
+            km, kp = (k - 1) % n_phi_, (k + 1) % n_phi_
+            Sm, S0, Sp = S_of(km), S_of(k), S_of(kp)
+            wm, w0, wp = wsum_of(km), wsum_of(k), wsum_of(kp)
+            sel = np.nonzero(plane_of_row == k)[0]
+            kd, rf, dp_ = kind[sel], ref[sel], dpl[sel]
+            m = kd == 0
+            vals[sel[m]] = sigma_ * eye[None] + (2.0 * beta_) * T[None] + (1.0 / 3.0) * (
+                0.5 * wm[rf[m]][:, None, None] * Sm[None] + w0[rf[m]][:, None, None] * S0[None] + 0.5 * wp[rf[m]][:, None, None] * Sp[None])
+            m = kd == 1
+            vals[sel[m]] = (-1.0 / 3.0) * (0.5 * w_k[km][rf[m]][:, None, None] * Sm[None] + w_k[k][rf[m]][:, None, None] * S0[None]
+                                           + 0.5 * w_k[kp][rf[m]][:, None, None] * Sp[None])
+            for dk, Sn, wn, kn in ((-1, Sm, wm, km), (1, Sp, wp, kp)):
+                m = (kd == 2) & (dp_ == dk)
+                vals[sel[m]] = (1.0 / 12.0) * (w0[rf[m]][:, None, None] * S0[None] + wn[rf[m]][:, None, None] * Sn[None]) - beta_ * T[None]
+                m = (kd == 3) & (dp_ == dk)
+                vals[sel[m]] = (-1.0 / 12.0) * (w_k[k][rf[m]][:, None, None] * S0[None] + w_k[kn][rf[m]][:, None, None] * Sn[None])
+    for k in range(n_phi_ if not prism_ else 0):
+        Sk = S_of(k)
+        wsum = wsum_of(k)
         sel = np.nonzero(plane_of_row == k)[0]
         kd, rf = kind[sel], ref[sel]
         d = sel[kd == 0]
@@ -224,6 +272,8 @@ def make_workload(name: str = "C0", *, mesh=None, n_phi=None, levels=None, sigma
         mate = np.searchsorted(key, cols[up] * n + rows[up])
         assert np.array_equal(key[mate], cols[up] * n + rows[up]), "pattern is not structurally symmetric"
         coef = np.where(kind[up] == 1, w_k[plane_of_row[up], ref[up]], beta_)
+        if prism_:
+            coef = np.where(kind[up] == 3, w_k[plane_of_row[up], ref[up]] / 6.0, coef)
         rng_n = _rng(seed_, 5)
         scale = delta_ / np.sqrt(b_)
         for s in range(0, up.shape[0], noise_chunk):

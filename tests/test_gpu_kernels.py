@@ -19,6 +19,8 @@ CASES = {
     "b5-generic-to-1-plane": dict(name="C0", mesh=(3, 8), n_phi=4, levels=3, b=5, seed=79),
     "b1": dict(name="C0", mesh=(3, 7), n_phi=6, levels=2, b=1, seed=80),
     "b36-nonaxi": dict(name="C3", mesh=(3, 10), n_phi=8, levels=3, seed=81),
+    # C3b recipe (21-block prism stencil on the fine level, plane-modulated), reduced
+    "b36-prism": dict(name="C3b", mesh=(3, 10), n_phi=8, levels=3, seed=88),
     # largest supported block (generic kernel; the batched inverse needs > 48 KB of shared memory) and a tiny one
     "b64-max-block": dict(name="C0", mesh=(2, 6), n_phi=4, levels=2, b=64, seed=86),
     "b2": dict(name="C0", mesh=(2, 5), n_phi=4, levels=3, b=2, seed=87),

@@ -212,3 +212,37 @@ def test_galerkin_kronecker_closed_form_at_delta_zero(golden):
     assert round(nnz / dofs / 36) == blocks and round(NNZ / N / 36) == blocks
     assert np.diff(Lc.row_ptr).max() == blocks
     assert np.diff(L.row_ptr).max() == 9
+
+
+# ---------------------------------------------------------------------------------------------- generator: prism stencil
+def test_prism_stencil_variant_closed_form_and_density(golden):
+    """C3b (Q16): the 21-block prism stencil on the fine level.  At delta = 0 and without plane modulation
+    A = sigma I + circ(1/6,2/3,1/6) (x) (L_w (x) S) + beta circ(-1,2,-1) (x) I (x) T; its interior rows hold the 21 blocks per
+    row of the paper's matrices (Table 5); it stays symmetric positive definite with the plane modulation."""
+    w = tiny(n_phi=4, b=3, delta=0.0, mesh=(3, 7), prism=True)
+    edges, wts = w.adj_w
+    Lw = np.zeros((w.n_pol, w.n_pol))
+    for (i, j), wij in zip(edges, wts):
+        Lw[i, i] += wij
+        Lw[j, j] += wij
+        Lw[i, j] -= wij
+        Lw[j, i] -= wij
+    n = w.n_pol * w.b
+    expect = w.sigma * np.eye(4 * n) + np.kron(circ(4, 1 / 6, 2 / 3, 1 / 6), np.kron(Lw, w.S)) + w.beta * np.kron(
+        circ(4, -1.0, 2.0, -1.0), np.kron(np.eye(w.n_pol), w.T))
+    got = dense_of(w)
+    assert np.abs(got - expect).max() <= 1e-13 * np.abs(expect).max()
+    dofs, nnz, N, NNZ, blocks = golden("nnz_per_row.txt")
+    assert np.diff(w.row_ptr).max() == blocks == 21
+    for kw in (dict(delta=0.0, nonaxisymmetric=True), dict(delta=0.15, nonaxisymmetric=True)):
+        wm = tiny(n_phi=4, b=3, mesh=(3, 7), prism=True, **kw)
+        A = dense_of(wm)
+        if kw["delta"] == 0.0:
+            assert np.abs(A - A.T).max() <= 1e-14 * np.abs(A).max()
+        assert np.linalg.eigvalsh(0.5 * (A + A.T)).min() >= 0.999 * wm.sigma       # noise is skew-symmetric
+        v = np.array([1.0, -2.0, 0.5])
+        if kw["delta"] == 0.0:
+            assert np.abs(A @ np.tile(v, wm.n_brows) - wm.sigma * np.tile(v, wm.n_brows)).max() <= 1e-12 * np.abs(A).max()
+    # SpMV of the oracle on the 21-block pattern
+    x = input_vector(w.n, 3)
+    assert np.abs(mg.spmv(level_of(w), x) - got @ x).max() <= 1e-13 * np.abs(got @ x).max()
