@@ -256,7 +256,7 @@ def cuda_arm(args):
     buildlib.build()
 
     t0 = time.perf_counter()
-    w = make_workload(args.workload)
+    w = make_workload(args.workload, **({"levels": args.levels} if args.levels > 0 else {}))
     gen_s = time.perf_counter() - t0
     rp, ci, va = binding.upload(w, dev)
     torch.cuda.synchronize()
@@ -453,6 +453,9 @@ def main():
                          "marked \"truncated\": true and is NOT a bench value")
     ap.add_argument("--smoother", choices=["chebyshev", "gmres"], default="chebyshev",
                     help="level smoother: PBJ-Chebyshev (default, the metric's configuration) or the paper's PBJ-GMRES (NEXT-1)")
+    ap.add_argument("--levels", type=int, default=0,
+                    help="override the number of MG levels of the workload (e.g. 5 on C1: coarsen to 1 plane as the paper does, "
+                         "PAPER.md:181); not the metric's configuration")
     ap.add_argument("--nu", type=int, default=0, help="smoothing steps pre and post (default: the library's 2)")
     ap.add_argument("--warmup-outer", type=int, default=4,
                     help="outer FGMRES iterations of each warm-up step (default 4, about 2.5 s on C1); 0 = complete solves")
