@@ -266,6 +266,8 @@ def cuda_arm(args):
         extra["smoother"] = 1
     if args.nu > 0:
         extra.update(nu_pre=args.nu, nu_post=args.nu)
+    if args.coarse_mode >= 0:
+        extra["coarse_mode"] = args.coarse_mode
     s = binding.Solver(rp, ci, va, w.b, w.n_pol, w.n_phi, w.levels, **extra)
     torch.cuda.synchronize()
     setup_s = time.perf_counter() - t0
@@ -405,7 +407,8 @@ def cuda_arm(args):
                 "dtype": "f64", "data": "synthetic",
                 "config": {"workload": w.name, "n_pol": w.n_pol, "n_phi": w.n_phi, "b": w.b, "levels": w.levels,
                            "unknowns": n, "nnzb": w.nnzb, "rtol": RTOL, "cycle": f"V({opt['nu_pre']},{opt['nu_post']}) " + ("PBJ-GMRES smoother (the paper's, PAPER.md:95)" if args.smoother == "gmres" else "PBJ-Chebyshev"),
-                           "coarsest": f"PBJ-GMRES({opt['coarse_restart']}) to {opt['coarse_rtol']:g}", "fgmres_restart": opt["restart"],
+                           "coarsest": ("direct (block-tridiagonal Schur inverses)" if opt["coarse_mode"] == 2 else
+                                        f"PBJ-GMRES({opt['coarse_restart']}) to {opt['coarse_rtol']:g}"), "fgmres_restart": opt["restart"],
                            "parallelism": "replicas only" if world > 1 else "1 GPU", "setup_s": setup_s, "refresh_s": refresh_s,
                            "l2": "inputs larger than L2 (every level's matrix >= 0.5 GB vs 126 MB L2)" if sizes[-1].matrix_bytes > 2.6e8
                            else "coarsest level fits L2: not an HBM-roofline workload",
@@ -456,6 +459,9 @@ def main():
     ap.add_argument("--levels", type=int, default=0,
                     help="override the number of MG levels of the workload (e.g. 5 on C1: coarsen to 1 plane as the paper does, "
                          "PAPER.md:181); not the metric's configuration")
+    ap.add_argument("--coarse-mode", type=int, default=-1,
+                    help="override the coarsest-level solver: 0 PBJ-GMRES to 1e-10 (the configs'; default), 2 direct "
+                         "(block-tridiagonal Schur inverses, NEXT-2); not the metric's configuration")
     ap.add_argument("--nu", type=int, default=0, help="smoothing steps pre and post (default: the library's 2)")
     ap.add_argument("--warmup-outer", type=int, default=4,
                     help="outer FGMRES iterations of each warm-up step (default 4, about 2.5 s on C1); 0 = complete solves")

@@ -63,7 +63,11 @@ typedef struct mg_options {
     double cheb_lo, cheb_hi; /* Chebyshev interval [cheb_lo, cheb_hi] * rho_est(D^-1 A); default 0.1, 1.1 */
     int eig_iters;           /* power iterations for rho_est; default 20 */
     int coarse_mode;         /* 0: PBJ-GMRES(coarse_restart) to coarse_rtol (default);
-                                1: coarse_fixed_sweeps Chebyshev-PBJ sweeps (a fixed polynomial: parity mode) */
+                                1: coarse_fixed_sweeps Chebyshev-PBJ sweeps (a fixed polynomial: parity mode);
+                                2: direct solve (the paper's LU on the coarsest level):
+                                   block rows ordered by BFS level sets => block tridiagonal with dense blocks; explicit
+                                   inverses of the Schur complements at setup/refresh, dense mat-vec streaming per solve.
+                                   Memory 4 * sum_k n_k^2 doubles: MG_ENOMEM if it does not fit */
     double coarse_rtol;      /* default 1e-10 (configs[1]) */
     int coarse_restart, coarse_maxit, coarse_fixed_sweeps; /* defaults 100, 20000, 8 (restart: DESIGN.md Q9) */
     int restart, maxit;      /* outer FGMRES restart length and iteration cap; defaults 100, 400

@@ -106,7 +106,7 @@ class Options:
     cheb_lo: float = 0.1
     cheb_hi: float = 1.1
     eig_iters: int = 20
-    coarse_mode: int = 0  # 0: PBJ-GMRES to coarse_rtol; 1: coarse_fixed_sweeps of Chebyshev-PBJ
+    coarse_mode: int = 0  # 0: PBJ-GMRES to coarse_rtol; 1: coarse_fixed_sweeps of Chebyshev-PBJ; 2: direct (sparse LU)
     coarse_rtol: float = 1e-10
     coarse_restart: int = 100
     coarse_maxit: int = 20000
@@ -360,6 +360,16 @@ def coarse_solve(H: Hierarchy, rhs: np.ndarray) -> np.ndarray:
         H.coarse_iters_last = o.coarse_fixed_sweeps
         H.coarse_iters_total += o.coarse_fixed_sweeps
         return chebyshev(L, rhs, None, o.coarse_fixed_sweeps)
+    if o.coarse_mode == 2:
+        # NEXT-2: the paper solves its coarsest level directly (LU).  The factorisation
+        # is a library primitive here (SuperLU through SciPy); the definition is e = A_c^-1 rhs.
+        if "coarse_lu" not in H.stats:
+            import scipy.sparse as sp
+            import scipy.sparse.linalg as spla
+            A = sp.bsr_matrix((L.vals, L.col_idx, L.row_ptr), shape=(L.n, L.n)).tocsc()
+            H.stats["coarse_lu"] = spla.splu(A)
+        H.coarse_iters_last = 0
+        return H.stats["coarse_lu"].solve(rhs)
     e, it, _, _ = fgmres(lambda v: spmv(L, v), lambda v: pbj_apply(L, v), rhs, None, o.coarse_rtol,
                          o.coarse_restart, o.coarse_maxit)
     H.coarse_iters_last = it

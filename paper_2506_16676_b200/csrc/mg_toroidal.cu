@@ -8,11 +8,13 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <queue>
 #include <string>
 #include <vector>
 
 #include "kernels_bsr.cuh"
 #include "kernels_bsr_tma.cuh"
+#include "kernels_direct.cuh"
 #include "kernels_setup.cuh"
 #include "kernels_vec.cuh"
 
@@ -70,6 +72,22 @@ struct Gmres {
     unsigned *orth_counter = nullptr;
 };
 
+// Direct solve of the coarsest level (kernels_direct.cuh): level-set ordering, dense blocks, explicit Schur inverses.
+struct DirectCoarse {
+    bool symbolic = false, numeric = false;
+    int nlev = 0;
+    std::vector<int> nk;        // dense dimension of every level set
+    std::vector<int> voff;      // offset of every level set in the permuted vector (scalars)
+    std::vector<double *> D, Lm, U, M;   // device; D becomes S^-1, M = L S_{k-1}^-1
+    int32_t *perm = nullptr, *inv = nullptr, *lev = nullptr, *off = nullptr;   // device
+    double **dD = nullptr, **dL = nullptr, **dU = nullptr;                     // device pointer tables
+    int64_t *rob = nullptr;     // block row of every stored block
+    double *zb = nullptr, *xb = nullptr, *tb = nullptr, *colp = nullptr;
+    int *bad = nullptr;
+    int maxn = 0;
+    int64_t bytes = 0;
+};
+
 }  // namespace
 
 struct mg_handle {
@@ -92,6 +110,7 @@ struct mg_handle {
     double *red_partial = nullptr, *red_out = nullptr;
     unsigned *red_counter = nullptr;
     Gmres coarse, outer;
+    DirectCoarse direct;
     std::vector<Gmres> smooth_g;         // per level: Arnoldi engine of the GMRES-PBJ smoother (opt.smoother = 1)
     const double *outer_vals = nullptr;  // values of the operator FGMRES solves with (mg_set_operator); NULL = level 0's
     double *coarse_ahat = nullptr;       // A D^-1 of the coarsest level as one block-CSR matrix (fused coarse GMRES)
@@ -608,9 +627,212 @@ int refresh_coarse_ahat(mg_handle *h) {
     return MG_OK;
 }
 
+// ------------------------------------------------------------------------------------------------ direct coarse solve
+// Symbolic part (once per hierarchy): BFS level sets of the coarsest level's block graph, permutation, dense storage.
+int direct_symbolic(mg_handle *h) {
+    Level &L = h->lev.back();
+    DirectCoarse &dc = h->direct;
+    const int b = h->b;
+    const int64_t n = L.n_brows;
+    if (n <= 0 || n > (int64_t)1 << 30) return MG_EINVAL;
+    if (L.h_row_ptr.empty()) {
+        L.h_row_ptr.resize((size_t)n + 1);
+        L.h_col_idx.resize((size_t)L.nnzb);
+        CU(cudaMemcpyAsync(L.h_row_ptr.data(), L.row_ptr, sizeof(int64_t) * (n + 1), cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaMemcpyAsync(L.h_col_idx.data(), L.col_idx, sizeof(int32_t) * L.nnzb, cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+    }
+    // BFS from `start`; returns the level of every block row (every component is appended after the previous ones)
+    auto bfs = [&](int64_t start, std::vector<int> &lvl) {
+        lvl.assign((size_t)n, -1);
+        int maxl = 0;
+        int64_t last = start;
+        std::queue<int64_t> q;
+        auto run = [&](int64_t s0, int l0) {
+            lvl[s0] = l0;
+            q.push(s0);
+            while (!q.empty()) {
+                const int64_t u = q.front();
+                q.pop();
+                last = u;
+                maxl = std::max(maxl, lvl[u]);
+                for (int64_t p = L.h_row_ptr[u]; p < L.h_row_ptr[u + 1]; ++p) {
+                    const int64_t v = L.h_col_idx[p];
+                    if (lvl[v] < 0) {
+                        lvl[v] = lvl[u] + 1;
+                        q.push(v);
+                    }
+                }
+            }
+        };
+        run(start, 0);
+        for (int64_t s0 = 0; s0 < n; ++s0)
+            if (lvl[s0] < 0) run(s0, maxl + 2);   // another component: its own level sets, never adjacent to the previous ones
+        return last;
+    };
+    std::vector<int> lvl;
+    const int64_t far = bfs(0, lvl);
+    bfs(far, lvl);   // pseudo-peripheral start: narrower level sets
+    // compress level numbers (gaps between components) and order rows by level
+    std::vector<int> used;
+    {
+        std::vector<int> sorted(lvl);
+        std::sort(sorted.begin(), sorted.end());
+        sorted.erase(std::unique(sorted.begin(), sorted.end()), sorted.end());
+        used = sorted;
+    }
+    dc.nlev = (int)used.size();
+    std::vector<int32_t> lev_of_old((size_t)n), perm((size_t)n), inv((size_t)n), lev_new((size_t)n), off((size_t)dc.nlev + 1, 0);
+    for (int64_t i = 0; i < n; ++i) lev_of_old[i] = (int32_t)(std::lower_bound(used.begin(), used.end(), lvl[i]) - used.begin());
+    for (int64_t i = 0; i < n; ++i) off[lev_of_old[i] + 1]++;
+    for (int k = 0; k < dc.nlev; ++k) off[k + 1] += off[k];
+    {
+        std::vector<int32_t> cur(off.begin(), off.end() - 1);
+        for (int64_t i = 0; i < n; ++i) {   // stable within a level set: ascending old index
+            const int32_t pnew = cur[lev_of_old[i]]++;
+            perm[pnew] = (int32_t)i;
+            inv[i] = pnew;
+            lev_new[pnew] = lev_of_old[i];
+        }
+    }
+    dc.nk.resize(dc.nlev);
+    dc.voff.assign(dc.nlev + 1, 0);
+    dc.maxn = 0;
+    int64_t bytes = 0;
+    for (int k = 0; k < dc.nlev; ++k) {
+        dc.nk[k] = (off[k + 1] - off[k]) * b;
+        dc.voff[k + 1] = dc.voff[k] + dc.nk[k];
+        dc.maxn = std::max(dc.maxn, dc.nk[k]);
+        bytes += (int64_t)sizeof(double) * dc.nk[k] * dc.nk[k];
+        if (k > 0) bytes += 2 * (int64_t)sizeof(double) * dc.nk[k] * dc.nk[k - 1];          // L and M
+        if (k + 1 < dc.nlev) bytes += (int64_t)sizeof(double) * dc.nk[k] * ((off[k + 2] - off[k + 1]) * b);
+    }
+    size_t free_b = 0, total_b = 0;
+    CU(cudaMemGetInfo(&free_b, &total_b));
+    if ((double)bytes > 0.8 * (double)free_b) return MG_ENOMEM;
+    dc.bytes = bytes;
+    dc.D.assign(dc.nlev, nullptr);
+    dc.Lm.assign(dc.nlev, nullptr);
+    dc.U.assign(dc.nlev, nullptr);
+    dc.M.assign(dc.nlev, nullptr);
+    for (int k = 0; k < dc.nlev; ++k) {
+        MG(dalloc_t(h, &dc.D[k], (size_t)dc.nk[k] * dc.nk[k]));
+        if (k > 0) {
+            MG(dalloc_t(h, &dc.Lm[k], (size_t)dc.nk[k] * dc.nk[k - 1]));
+            MG(dalloc_t(h, &dc.M[k], (size_t)dc.nk[k] * dc.nk[k - 1]));
+        }
+        if (k + 1 < dc.nlev) MG(dalloc_t(h, &dc.U[k], (size_t)dc.nk[k] * dc.nk[k + 1]));
+    }
+    MG(dalloc_t(h, &dc.perm, (size_t)n));
+    MG(dalloc_t(h, &dc.inv, (size_t)n));
+    MG(dalloc_t(h, &dc.lev, (size_t)n));
+    MG(dalloc_t(h, &dc.off, (size_t)dc.nlev + 1));
+    MG(dalloc_t(h, &dc.dD, (size_t)dc.nlev));
+    MG(dalloc_t(h, &dc.dL, (size_t)dc.nlev));
+    MG(dalloc_t(h, &dc.dU, (size_t)dc.nlev));
+    MG(dalloc_t(h, &dc.zb, (size_t)L.nvec + 2));
+    MG(dalloc_t(h, &dc.xb, (size_t)L.nvec + 2));
+    MG(dalloc_t(h, &dc.tb, (size_t)dc.maxn + 2));
+    MG(dalloc_t(h, &dc.colp, (size_t)dc.maxn + 2));
+    MG(dalloc_t(h, &dc.bad, 4));
+    CU(cudaMemcpyAsync(dc.perm, perm.data(), sizeof(int32_t) * n, cudaMemcpyHostToDevice, h->stream));
+    CU(cudaMemcpyAsync(dc.inv, inv.data(), sizeof(int32_t) * n, cudaMemcpyHostToDevice, h->stream));
+    CU(cudaMemcpyAsync(dc.lev, lev_new.data(), sizeof(int32_t) * n, cudaMemcpyHostToDevice, h->stream));
+    CU(cudaMemcpyAsync(dc.off, off.data(), sizeof(int32_t) * (dc.nlev + 1), cudaMemcpyHostToDevice, h->stream));
+    CU(cudaMemcpyAsync(dc.dD, dc.D.data(), sizeof(double *) * dc.nlev, cudaMemcpyHostToDevice, h->stream));
+    CU(cudaMemcpyAsync(dc.dL, dc.Lm.data(), sizeof(double *) * dc.nlev, cudaMemcpyHostToDevice, h->stream));
+    CU(cudaMemcpyAsync(dc.dU, dc.U.data(), sizeof(double *) * dc.nlev, cudaMemcpyHostToDevice, h->stream));
+    if (L.row_of_block != nullptr) dc.rob = L.row_of_block;
+    else {
+        MG(dalloc_t(h, &dc.rob, (size_t)std::max<int64_t>(L.nnzb, 1)));
+        LAUNCH(h, rows_of_blocks_kernel, grid_for(n, 256, 1 << 30), 256, 0, L.row_ptr, n, dc.rob);
+    }
+    CU(cudaStreamSynchronize(h->stream));   // the host vectors above are locals
+    dc.symbolic = true;
+    return MG_OK;
+}
+
+int dense_inverse_inplace(mg_handle *h, double *A, int n) {
+    DirectCoarse &dc = h->direct;
+    for (int p = 0; p < n; ++p) {
+        LAUNCH(h, gj_pivot_kernel, (n + 255) / 256, 256, 0, A, n, p, dc.colp, dc.bad);
+        LAUNCH(h, gj_update_kernel, dim3((n + 255) / 256, (n + 15) / 16), 256, 0, A, n, p, dc.colp);
+        LAUNCH(h, gj_finish_pivot_kernel, 1, 1, 0, A, n, p);
+    }
+    CU(cudaGetLastError());
+    return MG_OK;
+}
+int dense_gemm(mg_handle *h, const double *A, const double *B, const double *C0, double *C, int m, int n, int k, double alpha,
+               double beta) {
+    LAUNCH(h, dense_gemm_kernel, dim3((n + 31) / 32, (m + 31) / 32), 1024, 0, A, B, C0, C, m, n, k, alpha, beta);
+    CU(cudaGetLastError());
+    return MG_OK;
+}
+
+// Numeric part (setup and every refresh): assemble the dense blocks, then S_k^-1 and M_k = L_k S_{k-1}^-1.
+int direct_numeric(mg_handle *h) {
+    Level &L = h->lev.back();
+    DirectCoarse &dc = h->direct;
+    KindScope scope(h, L.index, MG_KIND_OTHER);
+    for (int k = 0; k < dc.nlev; ++k) {
+        CU(cudaMemsetAsync(dc.D[k], 0, sizeof(double) * (size_t)dc.nk[k] * dc.nk[k], h->stream));
+        if (k > 0) CU(cudaMemsetAsync(dc.Lm[k], 0, sizeof(double) * (size_t)dc.nk[k] * dc.nk[k - 1], h->stream));
+        if (k + 1 < dc.nlev) CU(cudaMemsetAsync(dc.U[k], 0, sizeof(double) * (size_t)dc.nk[k] * dc.nk[k + 1], h->stream));
+    }
+    CU(cudaMemsetAsync(dc.bad, 0, sizeof(int), h->stream));
+    DirectTables t{dc.inv, dc.lev, dc.off, dc.dD, dc.dL, dc.dU};
+    if (L.nnzb > 0) LAUNCH(h, direct_assemble_kernel, (unsigned)L.nnzb, 128, 0, dc.rob, L.col_idx, L.vals, h->b, t, dc.bad);
+    CU(cudaGetLastError());
+    for (int k = 0; k < dc.nlev; ++k) {
+        if (k > 0) {
+            MG(dense_gemm(h, dc.Lm[k], dc.D[k - 1], nullptr, dc.M[k], dc.nk[k], dc.nk[k - 1], dc.nk[k - 1], 1.0, 0.0));   // M = L S^-1
+            MG(dense_gemm(h, dc.M[k], dc.U[k - 1], dc.D[k], dc.D[k], dc.nk[k], dc.nk[k], dc.nk[k - 1], -1.0, 1.0));     // S = D - M U
+        }
+        MG(dense_inverse_inplace(h, dc.D[k], dc.nk[k]));
+    }
+    int bad = 0;
+    CU(cudaMemcpyAsync(&bad, dc.bad, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    if (bad == 1) return MG_EINVAL;      // a block outside the tridiagonal band: the pattern is not structurally symmetric
+    if (bad == 2) return MG_ESINGULAR;
+    dc.numeric = true;
+    return MG_OK;
+}
+
+// e = A_c^-1 rhs by block forward / backward substitution: dense mat-vec streaming, no host synchronisation.
+int direct_solve(mg_handle *h, const double *rhs, double *e) {
+    Level &L = h->lev.back();
+    DirectCoarse &dc = h->direct;
+    KindScope scope(h, L.index, MG_KIND_OTHER);
+    const int b = h->b;
+    LAUNCH(h, permute_blocks_kernel, grid_for(L.nvec, 256, 1 << 30), 256, 0, rhs, dc.zb, dc.perm, L.n_brows, b, 0);
+    for (int k = 1; k < dc.nlev; ++k)   // z_k -= M_k z_{k-1}
+        LAUNCH(h, dense_gemv_kernel, (dc.nk[k] + 7) / 8, 256, 0, dc.M[k], dc.zb + dc.voff[k - 1], dc.zb + dc.voff[k],
+               dc.zb + dc.voff[k], dc.nk[k], dc.nk[k - 1], -1.0);
+    for (int k = dc.nlev - 1; k >= 0; --k) {
+        const double *zk = dc.zb + dc.voff[k];
+        if (k + 1 < dc.nlev) {          // t = z_k - U_k x_{k+1}
+            LAUNCH(h, dense_gemv_kernel, (dc.nk[k] + 7) / 8, 256, 0, dc.U[k], dc.xb + dc.voff[k + 1], zk, dc.tb, dc.nk[k],
+                   dc.nk[k + 1], -1.0);
+            zk = dc.tb;
+        }
+        LAUNCH(h, dense_gemv_kernel, (dc.nk[k] + 7) / 8, 256, 0, dc.D[k], zk, (const double *)nullptr, dc.xb + dc.voff[k], dc.nk[k],
+               dc.nk[k], 1.0);
+    }
+    LAUNCH(h, permute_blocks_kernel, grid_for(L.nvec, 256, 1 << 30), 256, 0, dc.xb, e, dc.perm, L.n_brows, b, 1);
+    CU(cudaGetLastError());
+    return MG_OK;
+}
+
 // Solve A_{L-1} x = rhs on the coarsest level's own buffers (L.rhs -> L.x), zero guess.
 int coarse_solve_internal(mg_handle *h) {
     Level &L = h->lev.back();
+    if (h->opt.coarse_mode == 2) {
+        if (!h->direct.symbolic) MG(direct_symbolic(h));
+        if (!h->direct.numeric) MG(direct_numeric(h));
+        h->coarse_iters_last = 0;
+        return direct_solve(h, L.rhs, L.x);
+    }
     if (h->opt.coarse_mode == 1) {
         h->coarse_iters_last = h->opt.coarse_fixed_sweeps;
         h->coarse_iters_total += h->coarse_iters_last;
@@ -977,7 +1199,7 @@ size_t mg_sizeof_solve_info(void) { return sizeof(mg_solve_info); }
 static int validate_options(const mg_options &o) {
     if (o.nu_pre < 0 || o.nu_post < 0 || o.eig_iters < 1) return MG_EINVAL;
     if (!(o.cheb_lo > 0.0) || !(o.cheb_hi > o.cheb_lo)) return MG_EINVAL;
-    if (o.coarse_mode < 0 || o.coarse_mode > 1 || !(o.coarse_rtol > 0.0)) return MG_EINVAL;
+    if (o.coarse_mode < 0 || o.coarse_mode > 2 || !(o.coarse_rtol > 0.0)) return MG_EINVAL;
     if (o.coarse_restart < 1 || o.coarse_maxit < 1 || o.coarse_fixed_sweeps < 0) return MG_EINVAL;
     if (o.restart < 1 || o.maxit < 1 || o.block_layout != 0) return MG_EINVAL;
     if (o.kernel_variant < 0 || o.kernel_variant > 1) return MG_EINVAL;
@@ -1124,6 +1346,7 @@ int mg_update_values(mg_handle *h, const double *vals) {
         if (l + 1 < h->n_levels) MG(galerkin_numeric(h, l));
     }
     MG(refresh_coarse_ahat(h));
+    h->direct.numeric = false;   // the dense Schur inverses of the direct coarse solve are rebuilt on first use
     CU(cudaStreamSynchronize(h->stream));
     return MG_OK;
 }

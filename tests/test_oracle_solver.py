@@ -241,3 +241,20 @@ def test_full_solve_against_dense_lu_c0_shape():
     assert rel <= 1e-8 * (1 + 1e-6) and abs(rel - hist[-1]) <= 1e-11
     assert np.linalg.norm(x - xstar) <= np.linalg.cond(A) * 1e-8 * np.linalg.norm(xstar)
     assert all(h2 <= h1 * (1 + 1e-12) for h1, h2 in zip(hist, hist[1:]))  # GMRES residuals never increase
+
+
+def test_direct_coarse_mode_is_the_exact_coarse_solve():
+    """coarse_mode = 2 (NEXT-2: the paper's LU on the coarsest level) against dense LAPACK, and the
+    cycle with it against the dense multigrid operator (whose coarsest level is A_c^-1)."""
+    w = tiny(b=2, n_phi=8, levels=3)
+    H = hierarchy(w, coarse_mode=2)
+    mats = dense_levels(H)
+    Ac = mats[-1][0]
+    rc = input_vector(Ac.shape[0], 51)
+    e = mg.coarse_solve(H, rc)
+    assert np.abs(e - np.linalg.solve(Ac, rc)).max() <= 1e-11 * np.abs(e).max()
+    M = dense_cycle_operator(H, 0, mats)
+    r = input_vector(w.n, 52)
+    assert np.abs(mg.vcycle(H, r) - M @ r).max() <= 1e-10 * np.abs(M @ r).max()
+    x, it, conv, hist = mg.solve(H, w.rhs, 1e-8)
+    assert conv and np.linalg.norm(w.rhs - mats[0][0] @ x) <= 1.05e-8 * np.linalg.norm(w.rhs)
