@@ -328,7 +328,7 @@ def cuda_arm(args):
 
     # ---- roofline: a short event-bracketed pass (same inputs, a few outer iterations) gives mean kernel durations
     peak, peak_src = measured_peaks()
-    roof, detail, cpu, vcycle_roof = None, [], None, None
+    roof, detail, cpu, vcycle_roof, direct = None, [], None, None, None
     if rank == 0:
         s.update_options(maxit=min(opt["maxit"], 2))
         s.profile_reset()
@@ -387,6 +387,25 @@ def cuda_arm(args):
                                          "GBps": solve_bytes / t_dev / 1e9, "frac_of_measured_peak": solve_bytes / t_dev / 1e9 / peak,
                                          "frac_of_8TBs_nominal": solve_bytes / t_dev / 1e9 / 8000.0,
                                          "coarse_steps_per_cycle": info["coarse_iters_total"] / max(1, info["iters"])}}
+        # ---- the same solve with the paper's kind of coarsest-level solver (direct, NEXT-2): reported beside the metric,
+        # which keeps the configs' PBJ-GMRES coarse solve
+        direct = None
+        if opt["coarse_mode"] == 0 and args.max_outer <= 0 and not args.no_direct:
+            try:
+                s.update_options(coarse_mode=2)
+                t0d = time.perf_counter()
+                s.solve_host(rhs_h, x_h, rtol=RTOL)           # first call builds the dense Schur inverses
+                torch.cuda.synchronize()
+                first_s = time.perf_counter() - t0d
+                _, info_d = s.solve_host(rhs_h, x_h, rtol=RTOL)
+                direct = {"value": info_d["solve_ms"] / 1e3, "unit": UNIT, "outer_iters": info_d["iters"], "rel_res": info_d["rel_res"],
+                          "converged": info_d["converged"], "factorisation_s": max(0.0, first_s - info_d["solve_ms"] / 1e3),
+                          "what": "mg_options.coarse_mode = 2: block-tridiagonal direct solve of the coarsest level "
+                                  "(the paper solves its coarsest level by LU, PAPER.md:374-381); not the metric's configuration"}
+            except Exception as exc:   # e.g. not enough memory for the dense blocks
+                direct = {"unavailable": str(exc)}
+            finally:
+                s.update_options(coarse_mode=opt["coarse_mode"])
         # ---- oracle timed beside it (rank 0, N = 1 only)
         if world == 1 and not args.no_cpu_baseline:
             gbs, dt, threads, desc = oracle_sample(w, args.cpu_seconds)
@@ -417,7 +436,7 @@ def cuda_arm(args):
                            "outer_iters": info["iters"], "coarse_iters": info["coarse_iters_total"], "rel_res": info["rel_res"],
                            "max_abs_x": x_dev_check},
                 "e2e": {"value": t_e2e, "unit": UNIT, "h2d_bytes_per_step": 8 * n, "d2h_bytes_per_step": 8 * n},
-                "gpu_launches": launches, "clocks": clocks, "roofline": roof, "vcycle_roofline": vcycle_roof, "cpu_baseline": cpu,
+                "gpu_launches": launches, "clocks": clocks, "roofline": roof, "vcycle_roofline": vcycle_roof, "direct_coarse_solve": direct, "cpu_baseline": cpu,
                 "throughput": {"value": world / t_dev, "unit": "solves/s"}, "truncated": args.max_outer > 0,
                 "kernels": detail[:12]}
         print(json.dumps(line), flush=True)
@@ -451,6 +470,7 @@ def main():
     ap.add_argument("--workload", default="C1", help="C1 (the metric's config, default); C0, C2-16/32/64, C3, C3b for other configs")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="CPU time of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-direct", action="store_true", help="skip the extra solve with the direct coarsest-level solver")
     ap.add_argument("--max-outer", type=int, default=0,
                     help="profiling aid (ncu launch lists): cap the outer FGMRES iterations of every solve; the line is then "
                          "marked \"truncated\": true and is NOT a bench value")
