@@ -3,12 +3,14 @@
 //
 // The block rows of the coarsest level are ordered by the level sets of a breadth-first search of its block graph: every
 // block then couples only rows of the same or of adjacent level sets, i.e. the matrix is BLOCK TRIDIAGONAL with dense
-// blocks D_k (n_k x n_k), L_k (n_k x n_{k-1}), U_k (n_k x n_{k+1}).  Setup (off the solve path) forms the inverses of the
-// Schur complements explicitly,  S_0 = D_0,  M_k = L_k S_{k-1}^-1,  S_k = D_k - M_k U_{k-1},  and the solve is dense
-// mat-vec streaming (bandwidth bound, 3 n_k^2 doubles per level set):
-//      forward :  z_0 = b_0,             z_k = b_k - M_k z_{k-1}
-//      backward:  x_q = S_q^-1 z_q,      x_k = S_k^-1 (z_k - U_k x_{k+1})
-// All matrices are row-major FP64.
+// diagonal blocks D_k (n_k x n_k) and SPARSE off-diagonal blocks L_k (n_k x n_{k-1}), U_k (n_k x n_{k+1}), which stay in
+// the level's block-CSR storage.  Setup (off the solve path) forms the inverses of the Schur complements explicitly,
+//      S_0 = D_0,   S_k = D_k - (L_k S_{k-1}^-1) U_{k-1},
+// (only S_k^-1 is kept: sum_k n_k^2 doubles plus one n_k x n_{k-1} scratch) and the solve is dense mat-vec streaming
+// (bandwidth bound, 2 n_k^2 doubles per level set) interleaved with small sparse products:
+//      forward :  y_k = S_k^-1 (b_k - L_k y_{k-1})
+//      backward:  x_q = y_q,      x_k = y_k - S_k^-1 (U_k x_{k+1})
+// All dense matrices are row-major FP64.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -16,36 +18,112 @@
 namespace mgk {
 
 struct DirectTables {       // device arrays describing the level-set ordering
+    const int32_t *perm;    // [n_brows] block row at NEW position p
     const int32_t *inv;     // [n_brows] new position of block row I
     const int32_t *lev;     // [n_brows] level set of NEW position p
     const int32_t *off;     // [nlev + 1] first new position of every level set
-    double *const *D;       // [nlev] dense blocks
-    double *const *Lm;      // [nlev] (Lm[0] unused)
-    double *const *U;       // [nlev] (U[nlev-1] unused)
+    double *const *S;       // [nlev] dense diagonal blocks (D_k at assembly, then S_k, then S_k^-1)
 };
 
-// One CTA per stored block: scatter it into the dense block of its (level set of row, level set of column).
+// One CTA per stored block: the blocks inside a level set are scattered into its dense diagonal block.
 __global__ void __launch_bounds__(128) direct_assemble_kernel(const int64_t *__restrict__ row_of_block,
                                                               const int32_t *__restrict__ col_idx,
-                                                              const double *__restrict__ vals, const int b, const DirectTables t,
-                                                              int *__restrict__ bad) {
+                                                              const double *__restrict__ vals, const int b, const DirectTables t) {
     const int64_t p = blockIdx.x;
     const int pi = t.inv[row_of_block[p]], pj = t.inv[col_idx[p]];
-    const int li = t.lev[pi], lj = t.lev[pj];
-    double *dst;
-    if (lj == li) dst = t.D[li];
-    else if (lj == li - 1) dst = t.Lm[li];
-    else if (lj == li + 1) dst = t.U[li];
-    else {
-        if (threadIdx.x == 0) atomicExch(bad, 1);
-        return;
-    }
-    const int ncols = (t.off[lj + 1] - t.off[lj]) * b;
-    const size_t r0 = (size_t)(pi - t.off[li]) * b, c0 = (size_t)(pj - t.off[lj]) * b;
+    const int li = t.lev[pi];
+    if (t.lev[pj] != li) return;
+    double *dst = t.S[li];
+    const int ncols = (t.off[li + 1] - t.off[li]) * b;
+    const size_t r0 = (size_t)(pi - t.off[li]) * b, c0 = (size_t)(pj - t.off[li]) * b;
     const double *src = vals + (size_t)p * b * b;
     for (int e = threadIdx.x; e < b * b; e += blockDim.x) {
         const int r = e / b, c = e - r * b;
         dst[(r0 + r) * ncols + c0 + c] = src[e];
+    }
+}
+
+// Sparse off-diagonal product of one level set with an adjacent one (L_k or U_k), one warp per scalar row:
+//      out[local row] = (y0 or 0) + sign * sum_{u in list of the block row} A_{pos[u]} v[col[u] * b ...]
+// list_ptr is indexed by the NEW position of the block row (first = first new position of the level set), list_pos holds
+// positions in the block-CSR arrays and list_col the new position of the block column.  v is a whole vector in the
+// permuted numbering; y0 / out are local to the level set.
+__global__ void __launch_bounds__(128) direct_offdiag_kernel(const int64_t *__restrict__ list_ptr,
+                                                             const int64_t *__restrict__ list_pos,
+                                                             const int32_t *__restrict__ list_col,
+                                                             const double *__restrict__ vals, const int b, const int first,
+                                                             const int rows, const double *__restrict__ v,
+                                                             const double *__restrict__ y0, double *__restrict__ out,
+                                                             const double sign) {
+    const int row = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (row >= rows) return;
+    const int pl = row / b, r = row - pl * b;
+    const int64_t u0 = list_ptr[first + pl], u1 = list_ptr[first + pl + 1];
+    double acc = 0.0;
+    for (int64_t u = u0; u < u1; ++u) {
+        const double *a = vals + ((size_t)list_pos[u] * b + r) * b;
+        const double *x = v + (size_t)list_col[u] * b;
+        for (int c = lane; c < b; c += 32) acc = fma(a[c], x[c], acc);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (lane == 0) out[row] = (y0 != nullptr ? y0[row] : 0.0) + sign * acc;
+}
+
+// Setup: M (n_k x n_{k-1}) = L_k S_{k-1}^-1 with L_k read from the block-CSR storage.  grid (ceil(n_{k-1} / 128), block
+// rows of level set k); thread = one column of M, 4 scalar rows at a time.
+__global__ void __launch_bounds__(128) direct_lsinv_kernel(const int64_t *__restrict__ row_ptr,
+                                                           const int32_t *__restrict__ col_idx,
+                                                           const double *__restrict__ vals, const int b, const DirectTables t,
+                                                           const int k, const double *__restrict__ Sprev, const int nprev,
+                                                           double *__restrict__ M) {
+    const int64_t I = t.perm[t.off[k] + blockIdx.y];
+    const int c = blockIdx.x * 128 + threadIdx.x;
+    if (c >= nprev) return;
+    const int64_t p0 = row_ptr[I], p1 = row_ptr[I + 1];
+    const int first_prev = t.off[k - 1];
+    for (int r0 = 0; r0 < b; r0 += 4) {
+        double acc[4] = {0.0, 0.0, 0.0, 0.0};
+        for (int64_t p = p0; p < p1; ++p) {
+            const int pj = t.inv[col_idx[p]];
+            if (t.lev[pj] != k - 1) continue;
+            const double *a = vals + (size_t)p * b * b;
+            const double *s = Sprev + (size_t)(pj - first_prev) * b * nprev + c;
+            for (int q = 0; q < b; ++q) {
+                const double sv = s[(size_t)q * nprev];
+#pragma unroll
+                for (int i = 0; i < 4; ++i)
+                    if (r0 + i < b) acc[i] = fma(a[(r0 + i) * b + q], sv, acc[i]);
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+            if (r0 + i < b) M[((size_t)blockIdx.y * b + r0 + i) * nprev + c] = acc[i];
+    }
+}
+
+// Setup: S_k -= M U_{k-1}.  The blocks of U_{k-1} in block column C of level set k are listed (positions in the block-CSR
+// arrays) in ucsc_pos[ucsc_ptr[new position of C] ...].  grid (block columns of level set k, ceil(n_k / 32)).
+__global__ void __launch_bounds__(128) direct_schur_kernel(const int64_t *__restrict__ ucsc_ptr,
+                                                           const int64_t *__restrict__ ucsc_pos,
+                                                           const int64_t *__restrict__ row_of_block,
+                                                           const double *__restrict__ vals, const int b, const DirectTables t,
+                                                           const int k, const double *__restrict__ M, const int nprev,
+                                                           double *__restrict__ S, const int nk) {
+    const int cnew = t.off[k] + blockIdx.x;
+    const int first_prev = t.off[k - 1];
+    const int64_t u0 = ucsc_ptr[cnew], u1 = ucsc_ptr[cnew + 1];
+    for (int idx = threadIdx.x; idx < 32 * b; idx += blockDim.x) {
+        const int m = blockIdx.y * 32 + idx / b, cc = idx % b;
+        if (m >= nk) break;
+        double acc = 0.0;
+        for (int64_t u = u0; u < u1; ++u) {
+            const int64_t p = ucsc_pos[u];
+            const double *mrow = M + (size_t)m * nprev + (size_t)(t.inv[row_of_block[p]] - first_prev) * b;
+            const double *a = vals + (size_t)p * b * b + cc;
+            for (int q = 0; q < b; ++q) acc = fma(mrow[q], a[(size_t)q * b], acc);
+        }
+        S[(size_t)m * nk + (size_t)blockIdx.x * b + cc] -= acc;
     }
 }
 
@@ -56,79 +134,164 @@ __global__ void rows_of_blocks_kernel(const int64_t *__restrict__ row_ptr, const
     for (int64_t p = row_ptr[I]; p < row_ptr[I + 1]; ++p) rob[p] = I;
 }
 
-// ---- in-place Gauss-Jordan inverse without pivoting (the Schur complements inherit a positive definite symmetric part)
-// step p, part 1: save column p, scale row p
-__global__ void gj_pivot_kernel(double *__restrict__ A, const int n, const int p, double *__restrict__ colp, int *__restrict__ bad) {
-    const int j = blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= n) return;
-    const double piv = A[(size_t)p * n + p];
-    if (j == 0 && !(fabs(piv) > 0.0)) atomicExch(bad, 2);
-    const double d = 1.0 / piv;
-    colp[j] = (j == p) ? 0.0 : A[(size_t)j * n + p];   // column p (read) and row p (written) only meet in the pivot
-    if (j != p) A[(size_t)p * n + j] *= d;
+// ---- in-place BLOCKED Gauss-Jordan inverse without pivoting (the Schur complements inherit a positive definite symmetric
+// part).  Panel K = [p0, p0 + w), w <= 32, three launches per panel:
+//      1. Pinv = A[K,K]^-1                                           (one CTA, shared memory)
+//      2. C = A[:,K] saved;  A[K,J] = Pinv A[K,J] (J != K),  A[K,K] = Pinv;  R = the new A[K,:]
+//      3. A[I,J] = A[I,J] - C[I,:] R[:,J]  (I != K, J != K),   A[I,K] = -C[I,:] Pinv   (I != K)
+// which is the scalar elimination (scale row p, eliminate column p, column p becomes -colp / pivot) taken w pivots at a
+// time: the matrix is read and written n / w times instead of n times.
+constexpr int GJ_W = 32;
+
+__global__ void __launch_bounds__(GJ_W *GJ_W) gj_panel_inverse_kernel(const double *__restrict__ A, const int n, const int p0,
+                                                                       const int w, double *__restrict__ Pinv,
+                                                                       int *__restrict__ bad) {
+    __shared__ double s[GJ_W][GJ_W + 1];
+    const int j = threadIdx.x & (GJ_W - 1), i = threadIdx.x / GJ_W;
+    const bool in = i < w && j < w;
+    s[i][j] = in ? A[(size_t)(p0 + i) * n + p0 + j] : (i == j ? 1.0 : 0.0);
+    __syncthreads();
+    for (int p = 0; p < w; ++p) {
+        const double piv = s[p][p], colp = s[i][p], rowp = s[p][j], aij = s[i][j];
+        __syncthreads();
+        if (threadIdx.x == 0 && !(fabs(piv) > 0.0 && fabs(piv) < 1.0e300)) atomicExch(bad, 2);
+        const double d = 1.0 / piv;
+        double v;
+        if (i == p) v = (j == p) ? d : rowp * d;
+        else if (j == p) v = -colp * d;
+        else v = fma(-colp, rowp * d, aij);
+        s[i][j] = v;
+        __syncthreads();
+    }
+    if (in) Pinv[i * GJ_W + j] = s[i][j];
 }
-// step p, part 2: eliminate column p from every other row; column p becomes -colp * d, A[p][p] = d
-__global__ void __launch_bounds__(256) gj_update_kernel(double *__restrict__ A, const int n, const int p,
-                                                        const double *__restrict__ colp) {
+
+// one thread per column j of the row panel (and, as a row index, per row of the column panel that is saved)
+__global__ void __launch_bounds__(256) gj_row_panel_kernel(double *__restrict__ A, const int n, const int p0, const int w,
+                                                           const double *__restrict__ Pinv, double *__restrict__ C,
+                                                           double *__restrict__ R) {
+    __shared__ double sp[GJ_W][GJ_W + 1];
+    for (int e = threadIdx.x; e < GJ_W * GJ_W; e += 256) {
+        const int q = e / GJ_W, c = e - q * GJ_W;
+        sp[q][c] = (q < w && c < w) ? Pinv[e] : 0.0;
+    }
+    __syncthreads();
     const int j = blockIdx.x * 256 + threadIdx.x;
-    const int i0 = blockIdx.y * 16;
     if (j >= n) return;
-    const double d = 1.0 / A[(size_t)p * n + p];   // pivot itself is still untouched (j == p is skipped in part 1)
-    const double apj = A[(size_t)p * n + j];
-    for (int i = i0; i < i0 + 16 && i < n; ++i) {
-        if (i == p) continue;
-        const double f = colp[i];
-        if (j == p) A[(size_t)i * n + p] = -f * d;
-        else A[(size_t)i * n + j] = fma(-f, apj, A[(size_t)i * n + j]);
-    }
-}
-__global__ void gj_finish_pivot_kernel(double *__restrict__ A, const int n, const int p) {
-    A[(size_t)p * n + p] = 1.0 / A[(size_t)p * n + p];
-}
-
-// ---- C (m x n) = beta * C0 + alpha * A (m x k) * B (k x n), all row-major; 32 x 32 tiles in shared memory
-__global__ void __launch_bounds__(1024) dense_gemm_kernel(const double *__restrict__ A, const double *__restrict__ B,
-                                                          const double *__restrict__ C0, double *__restrict__ C, const int m,
-                                                          const int n, const int k, const double alpha, const double beta) {
-    __shared__ double As[32][33], Bs[32][33];
-    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
-    const int row = blockIdx.y * 32 + ty, col = blockIdx.x * 32 + tx;
-    double acc = 0.0;
-    for (int k0 = 0; k0 < k; k0 += 32) {
-        As[ty][tx] = (row < m && k0 + tx < k) ? A[(size_t)row * k + k0 + tx] : 0.0;
-        Bs[ty][tx] = (k0 + ty < k && col < n) ? B[(size_t)(k0 + ty) * n + col] : 0.0;
-        __syncthreads();
+    if (j < p0 || j >= p0 + w)   // rows outside the panel: save A[j, K] (rows inside are not used by step 3)
+        for (int q = 0; q < w; ++q) C[(size_t)j * GJ_W + q] = A[(size_t)j * n + p0 + q];
+    double out[GJ_W];
+    if (j >= p0 && j < p0 + w) {
 #pragma unroll
-        for (int q = 0; q < 32; ++q) acc = fma(As[ty][q], Bs[q][tx], acc);
-        __syncthreads();
+        for (int q = 0; q < GJ_W; ++q) out[q] = sp[q][j - p0];
+    } else {
+        double a[GJ_W];
+#pragma unroll
+        for (int q = 0; q < GJ_W; ++q) a[q] = q < w ? A[(size_t)(p0 + q) * n + j] : 0.0;
+#pragma unroll
+        for (int q = 0; q < GJ_W; ++q) {
+            double acc = 0.0;
+#pragma unroll
+            for (int c = 0; c < GJ_W; ++c) acc = fma(sp[q][c], a[c], acc);
+            out[q] = acc;
+        }
     }
-    if (row < m && col < n) C[(size_t)row * n + col] = (beta != 0.0 ? beta * C0[(size_t)row * n + col] : 0.0) + alpha * acc;
+#pragma unroll
+    for (int q = 0; q < GJ_W; ++q)
+        if (q < w) {
+            A[(size_t)(p0 + q) * n + j] = out[q];
+            R[(size_t)q * n + j] = out[q];
+        }
 }
 
-// ---- y = (y0 or 0) + sign * A x, A row-major rows x cols; one warp per row (the solve's only kernel: bandwidth bound)
+// rank-w update, 64 x 64 tile per CTA, 4 x 4 outputs per thread (rows ty + 16 ii, columns tx + 16 jj)
+__global__ void __launch_bounds__(256) gj_update_kernel(double *__restrict__ A, const int n, const int p0, const int w,
+                                                        const double *__restrict__ C, const double *__restrict__ R) {
+    __shared__ double Cs[64][GJ_W + 1], Rs[GJ_W][64];
+    const int i0 = blockIdx.y * 64, j0 = blockIdx.x * 64;
+    for (int e = threadIdx.x; e < 64 * GJ_W; e += 256) {
+        const int i = e / GJ_W, q = e - i * GJ_W;
+        const int gi = i0 + i;
+        Cs[i][q] = (gi < n && q < w && (gi < p0 || gi >= p0 + w)) ? C[(size_t)gi * GJ_W + q] : 0.0;
+    }
+    for (int e = threadIdx.x; e < GJ_W * 64; e += 256) {
+        const int q = e >> 6, j = e & 63;
+        Rs[q][j] = (q < w && j0 + j < n) ? R[(size_t)q * n + j0 + j] : 0.0;
+    }
+    __syncthreads();
+    const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+    double acc[4][4];
+#pragma unroll
+    for (int ii = 0; ii < 4; ++ii)
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj) acc[ii][jj] = 0.0;
+#pragma unroll 8
+    for (int q = 0; q < GJ_W; ++q) {
+        double c[4], r[4];
+#pragma unroll
+        for (int ii = 0; ii < 4; ++ii) c[ii] = Cs[ty + 16 * ii][q];
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj) r[jj] = Rs[q][tx + 16 * jj];
+#pragma unroll
+        for (int ii = 0; ii < 4; ++ii)
+#pragma unroll
+            for (int jj = 0; jj < 4; ++jj) acc[ii][jj] = fma(c[ii], r[jj], acc[ii][jj]);
+    }
+#pragma unroll
+    for (int ii = 0; ii < 4; ++ii) {
+        const int gi = i0 + ty + 16 * ii;
+        if (gi >= n || (gi >= p0 && gi < p0 + w)) continue;   // the rows of the panel are final after step 2
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj) {
+            const int gj = j0 + tx + 16 * jj;
+            if (gj >= n) continue;
+            double *dst = A + (size_t)gi * n + gj;
+            *dst = ((gj >= p0 && gj < p0 + w) ? 0.0 : *dst) - acc[ii][jj];
+        }
+    }
+}
+
+// ---- y = (y0 or 0) + sign * A x, A row-major rows x cols (the solve's dense kernel: bandwidth bound).  Two rows per CTA,
+// four warps per row (a quarter of the row each, partial sums combined in a fixed order): for the few thousand rows of a
+// level set this gives ~10 CTAs per SM in flight, so the SMs stay evenly loaded.
+constexpr int GEMV_ROWS = 2;
 __global__ void __launch_bounds__(256) dense_gemv_kernel(const double *__restrict__ A, const double *__restrict__ x,
                                                          const double *__restrict__ y0, double *__restrict__ y, const int rows,
                                                          const int cols, const double sign) {
-    const int row = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
-    if (row >= rows) return;
-    const double *a = A + (size_t)row * cols;
+    __shared__ double part[8];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int row = blockIdx.x * GEMV_ROWS + (warp >> 2), quarter = warp & 3;
     double acc0 = 0.0, acc1 = 0.0;
-    if ((cols & 1) == 0 && (reinterpret_cast<uintptr_t>(x) & 15) == 0 && (reinterpret_cast<uintptr_t>(a) & 15) == 0) {
-        const double2 *a2 = reinterpret_cast<const double2 *>(a);
-        const double2 *x2 = reinterpret_cast<const double2 *>(x);
-#pragma unroll 4
-        for (int c = lane; c < (cols >> 1); c += 32) {
-            const double2 av = a2[c], xv = x2[c];
-            acc0 = fma(av.x, xv.x, acc0);
-            acc1 = fma(av.y, xv.y, acc1);
+    if (row < rows) {
+        const double *a = A + (size_t)row * cols;
+        if ((cols & 1) == 0 && (reinterpret_cast<uintptr_t>(x) & 15) == 0 && (reinterpret_cast<uintptr_t>(a) & 15) == 0) {
+            const double2 *a2 = reinterpret_cast<const double2 *>(a);
+            const double2 *x2 = reinterpret_cast<const double2 *>(x);
+            const int n2 = cols >> 1;
+            const int c0 = (int)((int64_t)n2 * quarter / 4), c1 = (int)((int64_t)n2 * (quarter + 1) / 4);
+#pragma unroll 8
+            for (int c = c0 + lane; c < c1; c += 32) {
+                const double2 av = a2[c], xv = x2[c];
+                acc0 = fma(av.x, xv.x, acc0);
+                acc1 = fma(av.y, xv.y, acc1);
+            }
+        } else {
+            const int c0 = (int)((int64_t)cols * quarter / 4), c1 = (int)((int64_t)cols * (quarter + 1) / 4);
+            for (int c = c0 + lane; c < c1; c += 32) acc0 = fma(a[c], x[c], acc0);
         }
-    } else {
-        for (int c = lane; c < cols; c += 32) acc0 = fma(a[c], x[c], acc0);
     }
     double s = acc0 + acc1;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-    if (lane == 0) y[row] = (y0 != nullptr ? y0[row] : 0.0) + sign * s;
+    if (lane == 0) part[warp] = s;
+    __syncthreads();
+    if (threadIdx.x < GEMV_ROWS) {
+        const int r = blockIdx.x * GEMV_ROWS + threadIdx.x;
+        if (r < rows) {
+            const double t = (part[4 * threadIdx.x] + part[4 * threadIdx.x + 1]) + (part[4 * threadIdx.x + 2] + part[4 * threadIdx.x + 3]);
+            y[r] = (y0 != nullptr ? y0[r] : 0.0) + sign * t;
+        }
+    }
 }
 
 // block-row permutation of a vector: dst[new p] = src[perm[p]] (gather) or dst[perm[p]] = src[p] (scatter)

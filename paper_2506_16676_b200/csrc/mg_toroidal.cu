@@ -78,11 +78,16 @@ struct DirectCoarse {
     int nlev = 0;
     std::vector<int> nk;        // dense dimension of every level set
     std::vector<int> voff;      // offset of every level set in the permuted vector (scalars)
-    std::vector<double *> D, Lm, U, M;   // device; D becomes S^-1, M = L S_{k-1}^-1
+    std::vector<double *> S;    // device; D_k at assembly, then the Schur complement S_k, then S_k^-1
+    double *Mtmp = nullptr;     // scratch of the numeric phase: L_k S_{k-1}^-1
     int32_t *perm = nullptr, *inv = nullptr, *lev = nullptr, *off = nullptr;   // device
-    double **dD = nullptr, **dL = nullptr, **dU = nullptr;                     // device pointer tables
+    double **dS = nullptr;      // device pointer table
+    int64_t *ucsc_ptr = nullptr, *ucsc_pos = nullptr;   // blocks of U_{k-1} by block column (new numbering)
+    int64_t *od_ptr[2] = {nullptr, nullptr}, *od_pos[2] = {nullptr, nullptr};   // blocks of L_k (0) / U_k (1) by block row
+    int32_t *od_col[2] = {nullptr, nullptr};                                    // (new numbering) and their new columns
     int64_t *rob = nullptr;     // block row of every stored block
-    double *zb = nullptr, *xb = nullptr, *tb = nullptr, *colp = nullptr;
+    double *zb = nullptr, *yb = nullptr, *tb = nullptr;
+    double *pinv = nullptr, *cpanel = nullptr, *rpanel = nullptr;   // blocked Gauss-Jordan: pivot-block inverse, saved panels
     int *bad = nullptr;
     int maxn = 0;
     int64_t bytes = 0;
@@ -695,53 +700,97 @@ int direct_symbolic(mg_handle *h) {
             lev_new[pnew] = lev_of_old[i];
         }
     }
+    // every block must couple equal or adjacent level sets (true for a structurally symmetric pattern); the blocks of
+    // U_{k-1} (row in level set k-1, column in level set k) are listed by block column for the Schur update
+    std::vector<int64_t> ucsc_ptr((size_t)n + 1, 0), ucsc_pos;
+    for (int64_t i = 0; i < n; ++i)
+        for (int64_t p = L.h_row_ptr[i]; p < L.h_row_ptr[i + 1]; ++p) {
+            const int64_t j = L.h_col_idx[p];
+            const int d = lev_of_old[j] - lev_of_old[i];
+            if (d > 1 || d < -1) return MG_EINVAL;
+            if (d == 1) ucsc_ptr[inv[j] + 1]++;
+        }
+    for (int64_t i = 0; i < n; ++i) ucsc_ptr[i + 1] += ucsc_ptr[i];
+    ucsc_pos.resize((size_t)std::max<int64_t>(ucsc_ptr[n], 1));
+    {
+        std::vector<int64_t> cur(ucsc_ptr.begin(), ucsc_ptr.end() - 1);
+        for (int64_t i = 0; i < n; ++i)
+            for (int64_t p = L.h_row_ptr[i]; p < L.h_row_ptr[i + 1]; ++p) {
+                const int64_t j = L.h_col_idx[p];
+                if (lev_of_old[j] - lev_of_old[i] == 1) ucsc_pos[cur[inv[j]]++] = p;
+            }
+    }
+    // row-wise lists of the off-diagonal blocks for the solve: side 0 = L (column one level set down), 1 = U (one up)
+    std::vector<int64_t> od_ptr[2], od_pos[2];
+    std::vector<int32_t> od_col[2];
+    for (int side = 0; side < 2; ++side) {
+        const int want = side == 0 ? -1 : 1;
+        od_ptr[side].assign((size_t)n + 1, 0);
+        for (int64_t pn = 0; pn < n; ++pn) {
+            const int64_t i = perm[pn];
+            for (int64_t p = L.h_row_ptr[i]; p < L.h_row_ptr[i + 1]; ++p) {
+                const int64_t j = L.h_col_idx[p];
+                if (lev_of_old[j] - lev_of_old[i] != want) continue;
+                od_pos[side].push_back(p);
+                od_col[side].push_back(inv[j]);
+            }
+            od_ptr[side][pn + 1] = (int64_t)od_pos[side].size();
+        }
+        if (od_pos[side].empty()) {
+            od_pos[side].push_back(0);
+            od_col[side].push_back(0);
+        }
+    }
     dc.nk.resize(dc.nlev);
     dc.voff.assign(dc.nlev + 1, 0);
     dc.maxn = 0;
-    int64_t bytes = 0;
+    int64_t bytes = 0, mtmp = 1;
     for (int k = 0; k < dc.nlev; ++k) {
         dc.nk[k] = (off[k + 1] - off[k]) * b;
         dc.voff[k + 1] = dc.voff[k] + dc.nk[k];
         dc.maxn = std::max(dc.maxn, dc.nk[k]);
         bytes += (int64_t)sizeof(double) * dc.nk[k] * dc.nk[k];
-        if (k > 0) bytes += 2 * (int64_t)sizeof(double) * dc.nk[k] * dc.nk[k - 1];          // L and M
-        if (k + 1 < dc.nlev) bytes += (int64_t)sizeof(double) * dc.nk[k] * ((off[k + 2] - off[k + 1]) * b);
+        if (k > 0) mtmp = std::max(mtmp, (int64_t)dc.nk[k] * dc.nk[k - 1]);
     }
+    bytes += (int64_t)sizeof(double) * mtmp;
     size_t free_b = 0, total_b = 0;
     CU(cudaMemGetInfo(&free_b, &total_b));
-    if ((double)bytes > 0.8 * (double)free_b) return MG_ENOMEM;
+    if ((double)bytes > 0.9 * (double)free_b) return MG_ENOMEM;
     dc.bytes = bytes;
-    dc.D.assign(dc.nlev, nullptr);
-    dc.Lm.assign(dc.nlev, nullptr);
-    dc.U.assign(dc.nlev, nullptr);
-    dc.M.assign(dc.nlev, nullptr);
-    for (int k = 0; k < dc.nlev; ++k) {
-        MG(dalloc_t(h, &dc.D[k], (size_t)dc.nk[k] * dc.nk[k]));
-        if (k > 0) {
-            MG(dalloc_t(h, &dc.Lm[k], (size_t)dc.nk[k] * dc.nk[k - 1]));
-            MG(dalloc_t(h, &dc.M[k], (size_t)dc.nk[k] * dc.nk[k - 1]));
-        }
-        if (k + 1 < dc.nlev) MG(dalloc_t(h, &dc.U[k], (size_t)dc.nk[k] * dc.nk[k + 1]));
-    }
+    dc.S.assign(dc.nlev, nullptr);
+    for (int k = 0; k < dc.nlev; ++k) MG(dalloc_t(h, &dc.S[k], (size_t)dc.nk[k] * dc.nk[k]));
+    MG(dalloc_t(h, &dc.Mtmp, (size_t)mtmp));
     MG(dalloc_t(h, &dc.perm, (size_t)n));
     MG(dalloc_t(h, &dc.inv, (size_t)n));
     MG(dalloc_t(h, &dc.lev, (size_t)n));
     MG(dalloc_t(h, &dc.off, (size_t)dc.nlev + 1));
-    MG(dalloc_t(h, &dc.dD, (size_t)dc.nlev));
-    MG(dalloc_t(h, &dc.dL, (size_t)dc.nlev));
-    MG(dalloc_t(h, &dc.dU, (size_t)dc.nlev));
+    MG(dalloc_t(h, &dc.dS, (size_t)dc.nlev));
+    MG(dalloc_t(h, &dc.ucsc_ptr, (size_t)n + 1));
+    MG(dalloc_t(h, &dc.ucsc_pos, ucsc_pos.size()));
+    for (int side = 0; side < 2; ++side) {
+        MG(dalloc_t(h, &dc.od_ptr[side], (size_t)n + 1));
+        MG(dalloc_t(h, &dc.od_pos[side], od_pos[side].size()));
+        MG(dalloc_t(h, &dc.od_col[side], od_col[side].size()));
+        CU(cudaMemcpyAsync(dc.od_ptr[side], od_ptr[side].data(), sizeof(int64_t) * (n + 1), cudaMemcpyHostToDevice, h->stream));
+        CU(cudaMemcpyAsync(dc.od_pos[side], od_pos[side].data(), sizeof(int64_t) * od_pos[side].size(), cudaMemcpyHostToDevice,
+                           h->stream));
+        CU(cudaMemcpyAsync(dc.od_col[side], od_col[side].data(), sizeof(int32_t) * od_col[side].size(), cudaMemcpyHostToDevice,
+                           h->stream));
+    }
     MG(dalloc_t(h, &dc.zb, (size_t)L.nvec + 2));
-    MG(dalloc_t(h, &dc.xb, (size_t)L.nvec + 2));
+    MG(dalloc_t(h, &dc.yb, (size_t)L.nvec + 2));
     MG(dalloc_t(h, &dc.tb, (size_t)dc.maxn + 2));
-    MG(dalloc_t(h, &dc.colp, (size_t)dc.maxn + 2));
+    MG(dalloc_t(h, &dc.pinv, (size_t)GJ_W * GJ_W));
+    MG(dalloc_t(h, &dc.cpanel, (size_t)dc.maxn * GJ_W + 2));
+    MG(dalloc_t(h, &dc.rpanel, (size_t)dc.maxn * GJ_W + 2));
     MG(dalloc_t(h, &dc.bad, 4));
     CU(cudaMemcpyAsync(dc.perm, perm.data(), sizeof(int32_t) * n, cudaMemcpyHostToDevice, h->stream));
     CU(cudaMemcpyAsync(dc.inv, inv.data(), sizeof(int32_t) * n, cudaMemcpyHostToDevice, h->stream));
     CU(cudaMemcpyAsync(dc.lev, lev_new.data(), sizeof(int32_t) * n, cudaMemcpyHostToDevice, h->stream));
     CU(cudaMemcpyAsync(dc.off, off.data(), sizeof(int32_t) * (dc.nlev + 1), cudaMemcpyHostToDevice, h->stream));
-    CU(cudaMemcpyAsync(dc.dD, dc.D.data(), sizeof(double *) * dc.nlev, cudaMemcpyHostToDevice, h->stream));
-    CU(cudaMemcpyAsync(dc.dL, dc.Lm.data(), sizeof(double *) * dc.nlev, cudaMemcpyHostToDevice, h->stream));
-    CU(cudaMemcpyAsync(dc.dU, dc.U.data(), sizeof(double *) * dc.nlev, cudaMemcpyHostToDevice, h->stream));
+    CU(cudaMemcpyAsync(dc.dS, dc.S.data(), sizeof(double *) * dc.nlev, cudaMemcpyHostToDevice, h->stream));
+    CU(cudaMemcpyAsync(dc.ucsc_ptr, ucsc_ptr.data(), sizeof(int64_t) * (n + 1), cudaMemcpyHostToDevice, h->stream));
+    CU(cudaMemcpyAsync(dc.ucsc_pos, ucsc_pos.data(), sizeof(int64_t) * ucsc_pos.size(), cudaMemcpyHostToDevice, h->stream));
     if (L.row_of_block != nullptr) dc.rob = L.row_of_block;
     else {
         MG(dalloc_t(h, &dc.rob, (size_t)std::max<int64_t>(L.nnzb, 1)));
@@ -754,72 +803,73 @@ int direct_symbolic(mg_handle *h) {
 
 int dense_inverse_inplace(mg_handle *h, double *A, int n) {
     DirectCoarse &dc = h->direct;
-    for (int p = 0; p < n; ++p) {
-        LAUNCH(h, gj_pivot_kernel, (n + 255) / 256, 256, 0, A, n, p, dc.colp, dc.bad);
-        LAUNCH(h, gj_update_kernel, dim3((n + 255) / 256, (n + 15) / 16), 256, 0, A, n, p, dc.colp);
-        LAUNCH(h, gj_finish_pivot_kernel, 1, 1, 0, A, n, p);
+    for (int p0 = 0; p0 < n; p0 += GJ_W) {
+        const int w = std::min(GJ_W, n - p0);
+        LAUNCH(h, gj_panel_inverse_kernel, 1, GJ_W * GJ_W, 0, A, n, p0, w, dc.pinv, dc.bad);
+        LAUNCH(h, gj_row_panel_kernel, (n + 255) / 256, 256, 0, A, n, p0, w, dc.pinv, dc.cpanel, dc.rpanel);
+        LAUNCH(h, gj_update_kernel, dim3((n + 63) / 64, (n + 63) / 64), 256, 0, A, n, p0, w, dc.cpanel, dc.rpanel);
     }
-    CU(cudaGetLastError());
-    return MG_OK;
-}
-int dense_gemm(mg_handle *h, const double *A, const double *B, const double *C0, double *C, int m, int n, int k, double alpha,
-               double beta) {
-    LAUNCH(h, dense_gemm_kernel, dim3((n + 31) / 32, (m + 31) / 32), 1024, 0, A, B, C0, C, m, n, k, alpha, beta);
     CU(cudaGetLastError());
     return MG_OK;
 }
 
-// Numeric part (setup and every refresh): assemble the dense blocks, then S_k^-1 and M_k = L_k S_{k-1}^-1.
+// Numeric part (setup and every refresh): assemble the dense diagonal blocks, then S_k = D_k - (L_k S_{k-1}^-1) U_{k-1}
+// and its inverse, level set by level set.
 int direct_numeric(mg_handle *h) {
     Level &L = h->lev.back();
     DirectCoarse &dc = h->direct;
     KindScope scope(h, L.index, MG_KIND_OTHER);
-    for (int k = 0; k < dc.nlev; ++k) {
-        CU(cudaMemsetAsync(dc.D[k], 0, sizeof(double) * (size_t)dc.nk[k] * dc.nk[k], h->stream));
-        if (k > 0) CU(cudaMemsetAsync(dc.Lm[k], 0, sizeof(double) * (size_t)dc.nk[k] * dc.nk[k - 1], h->stream));
-        if (k + 1 < dc.nlev) CU(cudaMemsetAsync(dc.U[k], 0, sizeof(double) * (size_t)dc.nk[k] * dc.nk[k + 1], h->stream));
-    }
+    const int b = h->b;
+    for (int k = 0; k < dc.nlev; ++k) CU(cudaMemsetAsync(dc.S[k], 0, sizeof(double) * (size_t)dc.nk[k] * dc.nk[k], h->stream));
     CU(cudaMemsetAsync(dc.bad, 0, sizeof(int), h->stream));
-    DirectTables t{dc.inv, dc.lev, dc.off, dc.dD, dc.dL, dc.dU};
-    if (L.nnzb > 0) LAUNCH(h, direct_assemble_kernel, (unsigned)L.nnzb, 128, 0, dc.rob, L.col_idx, L.vals, h->b, t, dc.bad);
+    DirectTables t{dc.perm, dc.inv, dc.lev, dc.off, dc.dS};
+    if (L.nnzb > 0) LAUNCH(h, direct_assemble_kernel, (unsigned)L.nnzb, 128, 0, dc.rob, L.col_idx, L.vals, b, t);
     CU(cudaGetLastError());
     for (int k = 0; k < dc.nlev; ++k) {
         if (k > 0) {
-            MG(dense_gemm(h, dc.Lm[k], dc.D[k - 1], nullptr, dc.M[k], dc.nk[k], dc.nk[k - 1], dc.nk[k - 1], 1.0, 0.0));   // M = L S^-1
-            MG(dense_gemm(h, dc.M[k], dc.U[k - 1], dc.D[k], dc.D[k], dc.nk[k], dc.nk[k], dc.nk[k - 1], -1.0, 1.0));     // S = D - M U
+            const int nk = dc.nk[k], np = dc.nk[k - 1];
+            LAUNCH(h, direct_lsinv_kernel, dim3((np + 127) / 128, nk / b), 128, 0, L.row_ptr, L.col_idx, L.vals, b, t, k,
+                   dc.S[k - 1], np, dc.Mtmp);
+            LAUNCH(h, direct_schur_kernel, dim3(nk / b, (nk + 31) / 32), 128, 0, dc.ucsc_ptr, dc.ucsc_pos, dc.rob, L.vals, b, t, k,
+                   dc.Mtmp, np, dc.S[k], nk);
+            CU(cudaGetLastError());
         }
-        MG(dense_inverse_inplace(h, dc.D[k], dc.nk[k]));
+        MG(dense_inverse_inplace(h, dc.S[k], dc.nk[k]));
     }
     int bad = 0;
     CU(cudaMemcpyAsync(&bad, dc.bad, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
     CU(cudaStreamSynchronize(h->stream));
-    if (bad == 1) return MG_EINVAL;      // a block outside the tridiagonal band: the pattern is not structurally symmetric
     if (bad == 2) return MG_ESINGULAR;
     dc.numeric = true;
     return MG_OK;
 }
 
-// e = A_c^-1 rhs by block forward / backward substitution: dense mat-vec streaming, no host synchronisation.
+// e = A_c^-1 rhs by block forward / backward substitution: dense mat-vec streaming of the S_k^-1 interleaved with the
+// sparse off-diagonal products, no host synchronisation.
 int direct_solve(mg_handle *h, const double *rhs, double *e) {
     Level &L = h->lev.back();
     DirectCoarse &dc = h->direct;
     KindScope scope(h, L.index, MG_KIND_OTHER);
     const int b = h->b;
     LAUNCH(h, permute_blocks_kernel, grid_for(L.nvec, 256, 1 << 30), 256, 0, rhs, dc.zb, dc.perm, L.n_brows, b, 0);
-    for (int k = 1; k < dc.nlev; ++k)   // z_k -= M_k z_{k-1}
-        LAUNCH(h, dense_gemv_kernel, (dc.nk[k] + 7) / 8, 256, 0, dc.M[k], dc.zb + dc.voff[k - 1], dc.zb + dc.voff[k],
-               dc.zb + dc.voff[k], dc.nk[k], dc.nk[k - 1], -1.0);
-    for (int k = dc.nlev - 1; k >= 0; --k) {
+    for (int k = 0; k < dc.nlev; ++k) {   // y_k = S_k^-1 (z_k - L_k y_{k-1})
         const double *zk = dc.zb + dc.voff[k];
-        if (k + 1 < dc.nlev) {          // t = z_k - U_k x_{k+1}
-            LAUNCH(h, dense_gemv_kernel, (dc.nk[k] + 7) / 8, 256, 0, dc.U[k], dc.xb + dc.voff[k + 1], zk, dc.tb, dc.nk[k],
-                   dc.nk[k + 1], -1.0);
+        if (k > 0) {
+            LAUNCH(h, direct_offdiag_kernel, (dc.nk[k] + 3) / 4, 128, 0, dc.od_ptr[0], dc.od_pos[0], dc.od_col[0], L.vals, b,
+                   dc.voff[k] / b, dc.nk[k], dc.yb, zk, dc.tb, -1.0);
             zk = dc.tb;
         }
-        LAUNCH(h, dense_gemv_kernel, (dc.nk[k] + 7) / 8, 256, 0, dc.D[k], zk, (const double *)nullptr, dc.xb + dc.voff[k], dc.nk[k],
-               dc.nk[k], 1.0);
+        LAUNCH(h, dense_gemv_kernel, (dc.nk[k] + GEMV_ROWS - 1) / GEMV_ROWS, 256, 0, dc.S[k], zk, (const double *)nullptr, dc.yb + dc.voff[k],
+               dc.nk[k], dc.nk[k], 1.0);
     }
-    LAUNCH(h, permute_blocks_kernel, grid_for(L.nvec, 256, 1 << 30), 256, 0, dc.xb, e, dc.perm, L.n_brows, b, 1);
+    // x_q = y_q on the last level set, x_k = y_k - S_k^-1 (U_k x_{k+1}); the solution is built in place in yb
+    for (int k = dc.nlev - 2; k >= 0; --k) {
+        LAUNCH(h, direct_offdiag_kernel, (dc.nk[k] + 3) / 4, 128, 0, dc.od_ptr[1], dc.od_pos[1], dc.od_col[1], L.vals, b,
+               dc.voff[k] / b, dc.nk[k], dc.yb, (const double *)nullptr, dc.tb, 1.0);
+        LAUNCH(h, dense_gemv_kernel, (dc.nk[k] + GEMV_ROWS - 1) / GEMV_ROWS, 256, 0, dc.S[k], dc.tb, dc.yb + dc.voff[k], dc.yb + dc.voff[k], dc.nk[k],
+               dc.nk[k], -1.0);
+    }
+    LAUNCH(h, permute_blocks_kernel, grid_for(L.nvec, 256, 1 << 30), 256, 0, dc.yb, e, dc.perm, L.n_brows, b, 1);
     CU(cudaGetLastError());
     return MG_OK;
 }
