@@ -65,9 +65,11 @@ typedef struct mg_options {
     int coarse_mode;         /* 0: PBJ-GMRES(coarse_restart) to coarse_rtol (default);
                                 1: coarse_fixed_sweeps Chebyshev-PBJ sweeps (a fixed polynomial: parity mode);
                                 2: direct solve (the paper's LU on the coarsest level):
-                                   block rows ordered by BFS level sets => block tridiagonal with dense blocks; explicit
-                                   inverses of the Schur complements at setup/refresh, dense mat-vec streaming per solve.
-                                   Memory 4 * sum_k n_k^2 doubles: MG_ENOMEM if it does not fit */
+                                   block rows ordered by BFS level sets => block tridiagonal, dense diagonal blocks, sparse
+                                   off-diagonal blocks; explicit inverses of the Schur complements at setup/refresh (blocked
+                                   Gauss-Jordan), dense mat-vec streaming per solve.  Memory sum_k n_k^2 doubles (n_k = size
+                                   of level set k) plus one n_k x n_{k-1} scratch: MG_ENOMEM if it does not fit, MG_EINVAL
+                                   if the block pattern is not structurally symmetric */
     double coarse_rtol;      /* default 1e-10 (configs[1]) */
     int coarse_restart, coarse_maxit, coarse_fixed_sweeps; /* defaults 100, 20000, 8 (restart: DESIGN.md Q9) */
     int restart, maxit;      /* outer FGMRES restart length and iteration cap; defaults 100, 400
