@@ -56,9 +56,14 @@ __global__ void __launch_bounds__(128) direct_offdiag_kernel(const int64_t *__re
                                                              const double *__restrict__ y0, double *__restrict__ out,
                                                              const double sign) {
     const int row = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
-    if (row >= rows) return;
+    cudaTriggerProgrammaticLaunchCompletion();   // the dense mat-vec that follows may start prefetching its matrix
+    if (row >= rows) {
+        cudaGridDependencySynchronize();
+        return;
+    }
     const int pl = row / b, r = row - pl * b;
-    const int64_t u0 = list_ptr[first + pl], u1 = list_ptr[first + pl + 1];
+    const int64_t u0 = list_ptr[first + pl], u1 = list_ptr[first + pl + 1];   // setup data: independent of the chain
+    cudaGridDependencySynchronize();                                          // v, y0 come from the previous kernels
     double acc = 0.0;
     for (int64_t u = u0; u < u1; ++u) {
         const double *a = vals + ((size_t)list_pos[u] * b + r) * b;
@@ -255,6 +260,7 @@ __global__ void __launch_bounds__(256) gj_update_kernel(double *__restrict__ A, 
 // four warps per row (a quarter of the row each, partial sums combined in a fixed order): for the few thousand rows of a
 // level set this gives ~10 CTAs per SM in flight, so the SMs stay evenly loaded.
 constexpr int GEMV_ROWS = 2;
+constexpr int GEMV_PREFETCH = 8192;   // bytes of every quarter row prefetched into L2 before the dependency wait
 __global__ void __launch_bounds__(256) dense_gemv_kernel(const double *__restrict__ A, const double *__restrict__ x,
                                                          const double *__restrict__ y0, double *__restrict__ y, const int rows,
                                                          const int cols, const double sign) {
@@ -262,6 +268,15 @@ __global__ void __launch_bounds__(256) dense_gemv_kernel(const double *__restric
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int row = blockIdx.x * GEMV_ROWS + (warp >> 2), quarter = warp & 3;
     double acc0 = 0.0, acc1 = 0.0;
+    // Programmatic dependent launch: the kernels of one direct solve form a chain; A is setup data, so the start of this
+    // warp's part of the row is pulled into L2 while the previous kernel is still running, then wait for x / y0.
+    cudaTriggerProgrammaticLaunchCompletion();
+    if (row < rows) {
+        const char *a = reinterpret_cast<const char *>(A + (size_t)row * cols + (size_t)cols * quarter / 4);
+        const int bytes = min((int)(((size_t)cols * (quarter + 1) / 4 - (size_t)cols * quarter / 4) * sizeof(double)), GEMV_PREFETCH);
+        for (int o = lane * 128; o < bytes; o += 32 * 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(a + o));
+    }
+    cudaGridDependencySynchronize();
     if (row < rows) {
         const double *a = A + (size_t)row * cols;
         if ((cols & 1) == 0 && (reinterpret_cast<uintptr_t>(x) & 15) == 0 && (reinterpret_cast<uintptr_t>(a) & 15) == 0) {
@@ -298,6 +313,8 @@ __global__ void __launch_bounds__(256) dense_gemv_kernel(const double *__restric
 __global__ void permute_blocks_kernel(const double *__restrict__ src, double *__restrict__ dst, const int32_t *__restrict__ perm,
                                       const int64_t n_brows, const int b, const int scatter) {
     const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    cudaTriggerProgrammaticLaunchCompletion();
+    cudaGridDependencySynchronize();
     if (e >= n_brows * b) return;
     const int64_t p = e / b;
     const int c = (int)(e - p * b);

@@ -212,6 +212,30 @@ inline void prof_end(mg_handle *h, ProfPair &pp) {
         if (prof__) prof_end(h, pp__);                              \
         count_launch(h);                                            \
     } while (0)
+// Programmatic dependent launch (the kernel calls cudaGridDependencySynchronize() before it touches data of the previous
+// kernel in the stream): the launch latency and the prologue overlap the tail of that kernel.
+template <typename... KArgs, typename... Args>
+inline void launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args... args) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+#define LAUNCH_PDL(h, kern, grid, block, smem, ...)                                \
+    do {                                                                           \
+        ProfPair pp__;                                                             \
+        const bool prof__ = prof_begin(h, pp__);                                   \
+        launch_pdl(kern, dim3(grid), dim3(block), (smem), (h)->stream, __VA_ARGS__); \
+        if (prof__) prof_end(h, pp__);                                             \
+        count_launch(h);                                                           \
+    } while (0)
 struct KindScope {  // books the launches of one scope under (level, kind)
     mg_handle *h;
     int level0, kind0;
@@ -851,25 +875,25 @@ int direct_solve(mg_handle *h, const double *rhs, double *e) {
     DirectCoarse &dc = h->direct;
     KindScope scope(h, L.index, MG_KIND_OTHER);
     const int b = h->b;
-    LAUNCH(h, permute_blocks_kernel, grid_for(L.nvec, 256, 1 << 30), 256, 0, rhs, dc.zb, dc.perm, L.n_brows, b, 0);
+    LAUNCH_PDL(h, permute_blocks_kernel, grid_for(L.nvec, 256, 1 << 30), 256, 0, rhs, dc.zb, dc.perm, L.n_brows, b, 0);
     for (int k = 0; k < dc.nlev; ++k) {   // y_k = S_k^-1 (z_k - L_k y_{k-1})
         const double *zk = dc.zb + dc.voff[k];
         if (k > 0) {
-            LAUNCH(h, direct_offdiag_kernel, (dc.nk[k] + 3) / 4, 128, 0, dc.od_ptr[0], dc.od_pos[0], dc.od_col[0], L.vals, b,
+            LAUNCH_PDL(h, direct_offdiag_kernel, (dc.nk[k] + 3) / 4, 128, 0, dc.od_ptr[0], dc.od_pos[0], dc.od_col[0], L.vals, b,
                    dc.voff[k] / b, dc.nk[k], dc.yb, zk, dc.tb, -1.0);
             zk = dc.tb;
         }
-        LAUNCH(h, dense_gemv_kernel, (dc.nk[k] + GEMV_ROWS - 1) / GEMV_ROWS, 256, 0, dc.S[k], zk, (const double *)nullptr, dc.yb + dc.voff[k],
+        LAUNCH_PDL(h, dense_gemv_kernel, (dc.nk[k] + GEMV_ROWS - 1) / GEMV_ROWS, 256, 0, dc.S[k], zk, (const double *)nullptr, dc.yb + dc.voff[k],
                dc.nk[k], dc.nk[k], 1.0);
     }
     // x_q = y_q on the last level set, x_k = y_k - S_k^-1 (U_k x_{k+1}); the solution is built in place in yb
     for (int k = dc.nlev - 2; k >= 0; --k) {
-        LAUNCH(h, direct_offdiag_kernel, (dc.nk[k] + 3) / 4, 128, 0, dc.od_ptr[1], dc.od_pos[1], dc.od_col[1], L.vals, b,
+        LAUNCH_PDL(h, direct_offdiag_kernel, (dc.nk[k] + 3) / 4, 128, 0, dc.od_ptr[1], dc.od_pos[1], dc.od_col[1], L.vals, b,
                dc.voff[k] / b, dc.nk[k], dc.yb, (const double *)nullptr, dc.tb, 1.0);
-        LAUNCH(h, dense_gemv_kernel, (dc.nk[k] + GEMV_ROWS - 1) / GEMV_ROWS, 256, 0, dc.S[k], dc.tb, dc.yb + dc.voff[k], dc.yb + dc.voff[k], dc.nk[k],
+        LAUNCH_PDL(h, dense_gemv_kernel, (dc.nk[k] + GEMV_ROWS - 1) / GEMV_ROWS, 256, 0, dc.S[k], dc.tb, dc.yb + dc.voff[k], dc.yb + dc.voff[k], dc.nk[k],
                dc.nk[k], -1.0);
     }
-    LAUNCH(h, permute_blocks_kernel, grid_for(L.nvec, 256, 1 << 30), 256, 0, dc.yb, e, dc.perm, L.n_brows, b, 1);
+    LAUNCH_PDL(h, permute_blocks_kernel, grid_for(L.nvec, 256, 1 << 30), 256, 0, dc.yb, e, dc.perm, L.n_brows, b, 1);
     CU(cudaGetLastError());
     return MG_OK;
 }

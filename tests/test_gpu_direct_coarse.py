@@ -1,6 +1,6 @@
 """GPU parity of the direct coarsest-level solve (the paper's LU on the coarsest level,
-PAPER.md:374-381): ``coarse_mode = 2`` -- BFS level-set ordering, block-tridiagonal dense blocks, explicit Schur
-inverses -- against the oracle's sparse LU.  Both sides are exact solves, so they agree to cond(A_c) * eps."""
+PAPER.md:374-381): ``coarse_mode = 2`` -- BFS level-set ordering, block tridiagonal with dense diagonal and sparse
+off-diagonal blocks, explicit Schur inverses (blocked Gauss-Jordan) -- against the oracle's sparse LU.  Both sides are exact solves, so they agree to cond(A_c) * eps."""
 import numpy as np
 import pytest
 
@@ -16,6 +16,8 @@ CASES = {
     "b5-generic-to-1-plane": dict(name="C0", mesh=(3, 8), n_phi=4, levels=3, b=5, seed=79),
     "b36-3lev": dict(name="C0", mesh=(3, 10), n_phi=8, levels=3, seed=85),
     "b36-prism": dict(name="C3b", mesh=(3, 10), n_phi=8, levels=3, seed=88),
+    # level sets of ~1,100 scalars: many panels of the blocked inverse, several 64 x 64 update tiles, a ragged last one
+    "b36-wide-level-sets": dict(name="C0", mesh=(8, 24), n_phi=4, levels=2, seed=89),
 }
 
 
