@@ -48,6 +48,7 @@ __global__ void __launch_bounds__(128) direct_assemble_kernel(const int64_t *__r
 // list_ptr is indexed by the NEW position of the block row (first = first new position of the level set), list_pos holds
 // positions in the block-CSR arrays and list_col the new position of the block column.  v is a whole vector in the
 // permuted numbering; y0 / out are local to the level set.
+constexpr int OD_MAXE = 8;   // listed blocks per row held in registers (more: generic loop)
 __global__ void __launch_bounds__(128) direct_offdiag_kernel(const int64_t *__restrict__ list_ptr,
                                                              const int64_t *__restrict__ list_pos,
                                                              const int32_t *__restrict__ list_col,
@@ -63,12 +64,38 @@ __global__ void __launch_bounds__(128) direct_offdiag_kernel(const int64_t *__re
     }
     const int pl = row / b, r = row - pl * b;
     const int64_t u0 = list_ptr[first + pl], u1 = list_ptr[first + pl + 1];   // setup data: independent of the chain
-    cudaGridDependencySynchronize();                                          // v, y0 come from the previous kernels
+    const int ne = (int)(u1 - u0);
     double acc = 0.0;
-    for (int64_t u = u0; u < u1; ++u) {
-        const double *a = vals + ((size_t)list_pos[u] * b + r) * b;
-        const double *x = v + (size_t)list_col[u] * b;
-        for (int c = lane; c < b; c += 32) acc = fma(a[c], x[c], acc);
+    if (ne <= OD_MAXE && b <= 64) {
+        // the row of every listed block (setup data too) is in registers before the previous kernel has finished
+        double a0[OD_MAXE], a1[OD_MAXE];
+        int col[OD_MAXE];
+#pragma unroll
+        for (int i = 0; i < OD_MAXE; ++i) {
+            col[i] = 0;
+            a0[i] = a1[i] = 0.0;
+            if (i < ne) {
+                col[i] = list_col[u0 + i];
+                const double *a = vals + ((size_t)list_pos[u0 + i] * b + r) * b;
+                if (lane < b) a0[i] = a[lane];
+                if (lane + 32 < b) a1[i] = a[lane + 32];
+            }
+        }
+        cudaGridDependencySynchronize();   // v, y0 come from the previous kernels
+#pragma unroll
+        for (int i = 0; i < OD_MAXE; ++i)
+            if (i < ne) {
+                const double *x = v + (size_t)col[i] * b;
+                if (lane < b) acc = fma(a0[i], x[lane], acc);
+                if (lane + 32 < b) acc = fma(a1[i], x[lane + 32], acc);
+            }
+    } else {
+        cudaGridDependencySynchronize();
+        for (int64_t u = u0; u < u1; ++u) {
+            const double *a = vals + ((size_t)list_pos[u] * b + r) * b;
+            const double *x = v + (size_t)list_col[u] * b;
+            for (int c = lane; c < b; c += 32) acc = fma(a[c], x[c], acc);
+        }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
@@ -256,56 +283,83 @@ __global__ void __launch_bounds__(256) gj_update_kernel(double *__restrict__ A, 
     }
 }
 
-// ---- y = (y0 or 0) + sign * A x, A row-major rows x cols (the solve's dense kernel: bandwidth bound).  Two rows per CTA,
-// four warps per row (a quarter of the row each, partial sums combined in a fixed order): for the few thousand rows of a
-// level set this gives ~10 CTAs per SM in flight, so the SMs stay evenly loaded.
+// ---- y = (y0 or 0) + sign * A x, A row-major rows x cols (the solve's dense kernel: bandwidth bound).  Two consecutive rows
+// per CTA, walked together by all 256 threads (every step of the CTA reads 2 x 4 KB of consecutive matrix bytes, four
+// 128-bit loads per thread in flight per row); the 8 warp sums of a row are combined in a fixed order.  For the few
+// thousand rows of a level set this gives ~10 CTAs per SM, so the SMs stay evenly loaded.
 constexpr int GEMV_ROWS = 2;
-constexpr int GEMV_PREFETCH = 8192;   // bytes of every quarter row prefetched into L2 before the dependency wait
+constexpr int GEMV_PREFETCH = 32768;   // leading bytes of the CTA's rows prefetched into L2 before the dependency wait
 __global__ void __launch_bounds__(256) dense_gemv_kernel(const double *__restrict__ A, const double *__restrict__ x,
                                                          const double *__restrict__ y0, double *__restrict__ y, const int rows,
                                                          const int cols, const double sign) {
-    __shared__ double part[8];
+    __shared__ double part[GEMV_ROWS][8];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int row = blockIdx.x * GEMV_ROWS + (warp >> 2), quarter = warp & 3;
-    double acc0 = 0.0, acc1 = 0.0;
+    const int r0 = blockIdx.x * GEMV_ROWS;
+    const bool two = r0 + 1 < rows;
+    const double *a0 = A + (size_t)r0 * cols;
+    const double *a1 = two ? a0 + cols : a0;
     // Programmatic dependent launch: the kernels of one direct solve form a chain; A is setup data, so the start of this
-    // warp's part of the row is pulled into L2 while the previous kernel is still running, then wait for x / y0.
+    // CTA's rows is pulled into L2 while the previous kernel is still running, then wait for x / y0.
     cudaTriggerProgrammaticLaunchCompletion();
-    if (row < rows) {
-        const char *a = reinterpret_cast<const char *>(A + (size_t)row * cols + (size_t)cols * quarter / 4);
-        const int bytes = min((int)(((size_t)cols * (quarter + 1) / 4 - (size_t)cols * quarter / 4) * sizeof(double)), GEMV_PREFETCH);
-        for (int o = lane * 128; o < bytes; o += 32 * 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(a + o));
+    {
+        const char *base = reinterpret_cast<const char *>(a0);
+        const size_t bytes = min((size_t)cols * sizeof(double) * (two ? 2 : 1), (size_t)GEMV_PREFETCH);
+        for (size_t o = (size_t)threadIdx.x * 128; o < bytes; o += 256 * 128) asm volatile("prefetch.global.L2 [%0];" ::"l"(base + o));
     }
     cudaGridDependencySynchronize();
-    if (row < rows) {
-        const double *a = A + (size_t)row * cols;
-        if ((cols & 1) == 0 && (reinterpret_cast<uintptr_t>(x) & 15) == 0 && (reinterpret_cast<uintptr_t>(a) & 15) == 0) {
-            const double2 *a2 = reinterpret_cast<const double2 *>(a);
-            const double2 *x2 = reinterpret_cast<const double2 *>(x);
-            const int n2 = cols >> 1;
-            const int c0 = (int)((int64_t)n2 * quarter / 4), c1 = (int)((int64_t)n2 * (quarter + 1) / 4);
-#pragma unroll 8
-            for (int c = c0 + lane; c < c1; c += 32) {
-                const double2 av = a2[c], xv = x2[c];
-                acc0 = fma(av.x, xv.x, acc0);
-                acc1 = fma(av.y, xv.y, acc1);
+    double s0 = 0.0, s1 = 0.0, t0 = 0.0, t1 = 0.0;   // row 0: s0 + s1, row 1: t0 + t1
+    if ((cols & 1) == 0 && (reinterpret_cast<uintptr_t>(x) & 15) == 0 && (reinterpret_cast<uintptr_t>(A) & 15) == 0) {
+        const double2 *p0 = reinterpret_cast<const double2 *>(a0);
+        const double2 *p1 = reinterpret_cast<const double2 *>(a1);
+        const double2 *x2 = reinterpret_cast<const double2 *>(x);
+        const int n2 = cols >> 1;
+        int c = threadIdx.x;
+        for (; c + 768 < n2; c += 1024) {
+            double2 u[4], v[4], xv[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) u[i] = p0[c + 256 * i];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) v[i] = p1[c + 256 * i];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) xv[i] = x2[c + 256 * i];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                s0 = fma(u[i].x, xv[i].x, s0);
+                s1 = fma(u[i].y, xv[i].y, s1);
+                t0 = fma(v[i].x, xv[i].x, t0);
+                t1 = fma(v[i].y, xv[i].y, t1);
             }
-        } else {
-            const int c0 = (int)((int64_t)cols * quarter / 4), c1 = (int)((int64_t)cols * (quarter + 1) / 4);
-            for (int c = c0 + lane; c < c1; c += 32) acc0 = fma(a[c], x[c], acc0);
+        }
+        for (; c < n2; c += 256) {
+            const double2 u = p0[c], v = p1[c], xv = x2[c];
+            s0 = fma(u.x, xv.x, s0);
+            s1 = fma(u.y, xv.y, s1);
+            t0 = fma(v.x, xv.x, t0);
+            t1 = fma(v.y, xv.y, t1);
+        }
+    } else {
+        for (int c = threadIdx.x; c < cols; c += 256) {
+            const double xv = x[c];
+            s0 = fma(a0[c], xv, s0);
+            t0 = fma(a1[c], xv, t0);
         }
     }
-    double s = acc0 + acc1;
+    double s = s0 + s1, t = t0 + t1;
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-    if (lane == 0) part[warp] = s;
+    for (int o = 16; o > 0; o >>= 1) {
+        s += __shfl_xor_sync(0xffffffffu, s, o);
+        t += __shfl_xor_sync(0xffffffffu, t, o);
+    }
+    if (lane == 0) {
+        part[0][warp] = s;
+        part[1][warp] = t;
+    }
     __syncthreads();
-    if (threadIdx.x < GEMV_ROWS) {
-        const int r = blockIdx.x * GEMV_ROWS + threadIdx.x;
-        if (r < rows) {
-            const double t = (part[4 * threadIdx.x] + part[4 * threadIdx.x + 1]) + (part[4 * threadIdx.x + 2] + part[4 * threadIdx.x + 3]);
-            y[r] = (y0 != nullptr ? y0[r] : 0.0) + sign * t;
-        }
+    if (threadIdx.x < GEMV_ROWS && r0 + (int)threadIdx.x < rows) {
+        const double *q = part[threadIdx.x];
+        const double sum = ((q[0] + q[1]) + (q[2] + q[3])) + ((q[4] + q[5]) + (q[6] + q[7]));
+        const int r = r0 + threadIdx.x;
+        y[r] = (y0 != nullptr ? y0[r] : 0.0) + sign * sum;
     }
 }
 
