@@ -169,6 +169,12 @@ int mg_prolong_add(mg_handle *h, int level, const double *e_coarse, double *x_fi
 /* Coarsest-level solve A_{L-1} e = r from a zero guess (mode per options); iters may be NULL. Synchronises. */
 int mg_coarse_solve(mg_handle *h, const double *r, double *e, int *iters);
 
+/* Direct coarsest-level solve (coarse_mode = 2), after its first use: number of BFS level sets, bytes of the dense Schur
+ * inverses (sum_k n_k^2 doubles), bytes of the off-diagonal blocks L_k, U_k read per solve, widest level set (scalars) and
+ * whether the persistent cooperative kernel is in use (else the launch chain).  One solve streams 2 * dense_bytes +
+ * offdiag_bytes.  Any out pointer may be NULL.  MG_EINVAL before the first direct solve. */
+int mg_direct_info(mg_handle *h, int *level_sets, int64_t *dense_bytes, int64_t *offdiag_bytes, int *max_n, int *persistent);
+
 /* Borrowed DEVICE pointers and sizes of one level (any out pointer may be NULL). */
 int mg_get_level(mg_handle *h, int level, int64_t *n_brows, int64_t *nnzb, const int64_t **row_ptr,
                  const int32_t **col_idx, const double **vals, const double **dinv, double *rho_est,
@@ -190,7 +196,8 @@ int mg_set_cheb_bounds(mg_handle *h, int level, double lam_min, double lam_max);
 #define MG_KIND_ORTH 7      /* (F)GMRES dots / axpys / Givens bookkeeping */
 #define MG_KIND_OTHER 8
 #define MG_KIND_CYCLE 9     /* one whole coarsest-level GMRES restart cycle in a single persistent kernel */
-#define MG_KIND_COUNT 10
+#define MG_KIND_DIRECT 10   /* direct coarsest-level solve: the persistent cooperative kernel (or its launch-chain fallback) */
+#define MG_KIND_COUNT 11
 #define MG_PROFILE_MAX_LEVELS 32
 /* Launches are always counted per (level, kind).  on != 0 additionally brackets every kernel launch with a
  * CUDA event pair on the stream and books its duration; CUDA-graph replay is bypassed while that is on. */

@@ -13,7 +13,7 @@ import os
 from . import buildlib
 
 MG_OK, MG_EINVAL, MG_ENOMEM, MG_ESINGULAR, MG_ECUDA = 0, -1, -2, -3, -4
-KIND_NAMES = ("spmv", "resid", "sweep", "sweep_nod", "pbj", "restrict", "prolong", "orth", "other", "cycle")
+KIND_NAMES = ("spmv", "resid", "sweep", "sweep_nod", "pbj", "restrict", "prolong", "orth", "other", "cycle", "direct")
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
 FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
@@ -53,6 +53,7 @@ SYMBOLS = {
     "mg_restrict": (_I, [_VP, _I, _VP, _VP]),
     "mg_prolong_add": (_I, [_VP, _I, _VP, _VP]),
     "mg_coarse_solve": (_I, [_VP, _VP, _VP, C.POINTER(_I)]),
+    "mg_direct_info": (_I, [_VP, C.POINTER(_I), C.POINTER(_I64), C.POINTER(_I64), C.POINTER(_I), C.POINTER(_I)]),
     "mg_get_level": (_I, [_VP, _I, C.POINTER(_I64), C.POINTER(_I64), C.POINTER(_VP), C.POINTER(_VP), C.POINTER(_VP),
                           C.POINTER(_VP), C.POINTER(_D), C.POINTER(_D), C.POINTER(_D)]),
     "mg_copy_level_to_host": (_I, [_VP, _I, _VP, _VP, _VP, _VP]),
@@ -263,6 +264,14 @@ class Solver:
         _chk(lib().mg_coarse_solve(self._h, _ptr(r, torch.float64), _ptr(e, torch.float64), C.byref(it)),
              "mg_coarse_solve")
         return e, it.value
+
+    def direct_info(self) -> dict:
+        """Sizes of the direct coarsest-level solve (after its first use)."""
+        ls, mx, pers = C.c_int(), C.c_int(), C.c_int()
+        dense, od = C.c_int64(), C.c_int64()
+        _chk(lib().mg_direct_info(self._h, C.byref(ls), C.byref(dense), C.byref(od), C.byref(mx), C.byref(pers)), "mg_direct_info")
+        return dict(level_sets=ls.value, dense_bytes=dense.value, offdiag_bytes=od.value, max_n=mx.value,
+                    persistent=bool(pers.value), bytes_per_solve=2 * dense.value + od.value)
 
     def get_level(self, level: int) -> dict:
         """Sizes, Chebyshev bounds and (as torch views of the library's device memory) the level's arrays."""

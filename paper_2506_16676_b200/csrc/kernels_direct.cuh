@@ -53,9 +53,9 @@ __global__ void __launch_bounds__(128) direct_offdiag_kernel(const int64_t *__re
                                                              const int64_t *__restrict__ list_pos,
                                                              const int32_t *__restrict__ list_col,
                                                              const double *__restrict__ vals, const int b, const int first,
-                                                             const int rows, const double *__restrict__ v,
-                                                             const double *__restrict__ y0, double *__restrict__ out,
-                                                             const double sign) {
+                                                             const int rows, const double *v, const double *y0, double *out,
+                                                             const double sign) {   // v, y0, out: written by the preceding
+                                                                                    // kernels of the chain -> no __restrict__
     const int row = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
     cudaTriggerProgrammaticLaunchCompletion();   // the dense mat-vec that follows may start prefetching its matrix
     if (row >= rows) {
@@ -289,9 +289,9 @@ __global__ void __launch_bounds__(256) gj_update_kernel(double *__restrict__ A, 
 // thousand rows of a level set this gives ~10 CTAs per SM, so the SMs stay evenly loaded.
 constexpr int GEMV_ROWS = 2;
 constexpr int GEMV_PREFETCH = 32768;   // leading bytes of the CTA's rows prefetched into L2 before the dependency wait
-__global__ void __launch_bounds__(256) dense_gemv_kernel(const double *__restrict__ A, const double *__restrict__ x,
-                                                         const double *__restrict__ y0, double *__restrict__ y, const int rows,
-                                                         const int cols, const double sign) {
+__global__ void __launch_bounds__(256) dense_gemv_kernel(const double *__restrict__ A, const double *x, const double *y0, double *y,
+                                                         const int rows, const int cols, const double sign) {   // x, y0, y: chain data
+                                                                                    // (y0 may alias y): no __restrict__
     __shared__ double part[GEMV_ROWS][8];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int r0 = blockIdx.x * GEMV_ROWS;
@@ -364,7 +364,7 @@ __global__ void __launch_bounds__(256) dense_gemv_kernel(const double *__restric
 }
 
 // block-row permutation of a vector: dst[new p] = src[perm[p]] (gather) or dst[perm[p]] = src[p] (scatter)
-__global__ void permute_blocks_kernel(const double *__restrict__ src, double *__restrict__ dst, const int32_t *__restrict__ perm,
+__global__ void permute_blocks_kernel(const double *src, double *dst, const int32_t *__restrict__ perm,
                                       const int64_t n_brows, const int b, const int scatter) {
     const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     cudaTriggerProgrammaticLaunchCompletion();
@@ -374,6 +374,412 @@ __global__ void permute_blocks_kernel(const double *__restrict__ src, double *__
     const int c = (int)(e - p * b);
     if (scatter) dst[(int64_t)perm[p] * b + c] = src[e];
     else dst[e] = src[(int64_t)perm[p] * b + c];
+}
+
+
+// ================================================================================================ persistent direct solve
+// ONE cooperative launch per coarsest-level direct solve instead of a chain of ~4 launches per level set.
+//
+//   * grid = one CTA per SM, co-resident (cooperative launch); CTA c owns the contiguous rows [n_k c/G, n_k (c+1)/G) of
+//     every level set k: of the dense inverse S_k^-1 (a contiguous span of the row-major matrix) and of the off-diagonal
+//     block rows L_k / U_k, which the numeric phase packs row by row into a padded (ELL) array in the level-set ordering;
+//   * hence the whole matrix stream of a solve (forward sweep k = 0..q, backward sweep k = q-1..0) is STATIC and contiguous
+//     per CTA and step: one producer warp walks it from start to end with 1-D bulk async copies (TMA engine, SASS UBLKCP)
+//     into a shared-memory ring of DS_SEG-double stages, gated only by the ring's "empty" barriers, and asks for the
+//     stream of the NEXT step to be prefetched into L2 (cp.async.bulk.prefetch.L2) -- a step has four dependent global
+//     round trips (y written -> gathered, t written -> read) of 1-2 us each under load, during which HBM keeps streaming;
+//   * 7 consumer warps per CTA.  Step of level set k:  (A) t = z_k - L_k y_{k-1} (forward) or t = U_k x_{k+1} (backward)
+//     for the CTA's rows, block rows out of the ring, only the gathered y / x values come from global memory;  grid
+//     barrier;  (B) every CTA copies t (n_k doubles) into shared memory and its warps multiply the CTA's rows of S_k^-1
+//     out of the ring (one row per warp at a time, 128-bit shared-memory reads, fixed summation order), writing y_k / x_k;
+//     grid barrier.  The permutation of the right-hand side and of the solution rides in (A) and (B).
+// Requirements (checked by the host, otherwise the launch chain above is used): b even (16-byte aligned rows for the bulk
+// copies), b <= 64, at most DS_MAXNE listed blocks per block row and side, max n_k doubles + DS_PL ring stages fit the
+// shared memory.
+constexpr int DS_SEG = 1024;            // doubles per ring stage (8 KB)
+constexpr int DS_WARPS = 7;             // consumer warps (+ 1 producer warp = 8: register allocation is per 4 warps)
+constexpr int DS_THREADS = (DS_WARPS + 1) * 32;
+constexpr int DS_PL = 16;               // producer lanes issuing copies in parallel
+constexpr int DS_MAXNE = 16;            // listed blocks per block row and side (ELL width); DS_MAXNE * 64 <= DS_SEG
+constexpr int DS_TPR = 8;               // threads per scalar row in the off-diagonal phase
+constexpr int DS_XCH = 32;              // gathered values a thread keeps in flight
+constexpr int DS_LOOKAHEAD = 48;        // stages (8 KB each, per CTA) the L2 prefetch runs ahead of the shared-memory ring
+constexpr int DS_NCOL = 8;              // column indices of the coming step's row a thread prefetches into registers
+struct DirectLevel {
+    const double *S;        // S_k^-1, row-major n x n
+    int n;                  // scalars in the level set
+    int first;              // first NEW block position of the level set (scalar offset = first * b)
+    long long ell_off[2];   // offset (doubles) of the level set's packed off-diagonal rows, side 0 = L_k, 1 = U_k
+    int ne[2];              // ELL width of the level set per side (0: no blocks)
+};
+struct DirectSolveArgs {
+    const DirectLevel *lv;   // [nlev]
+    int nlev, b;
+    const double *ell;       // packed off-diagonal rows: [scalar row][ne][b]
+    const int32_t *ell_col;  // [side][new block row][DS_MAXNE] new block column or -1
+    const int32_t *perm;     // block row at NEW position p
+    const double *rhs;       // [n] natural ordering
+    double *e;               // [n] natural ordering (solution)
+    double *yb, *tb;         // [n] permuted work vectors, [max n_k]
+    unsigned *bar;           // grid barrier counter, zero at launch
+    int64_t n_brows;
+    int stages, tcap;        // ring stages, capacity of the shared-memory copy of t (doubles)
+};
+inline size_t direct_smem_bytes(int stages, int tcap) {
+    return sizeof(double) * ((size_t)stages * DS_SEG + (size_t)tcap) + sizeof(uint64_t) * 2 * (size_t)stages + sizeof(int) * (size_t)stages + 64;
+}
+
+// Numeric phase: pack the listed off-diagonal blocks of every block row (side 0 / 1) into the ELL array of its level set.
+// grid (n_brows, 2); lev_ne / lev_off: [nlev][2].
+__global__ void __launch_bounds__(128) direct_pack_ell_kernel(const int64_t *__restrict__ od_ptr0, const int64_t *__restrict__ od_pos0,
+                                                              const int32_t *__restrict__ od_col0, const int64_t *__restrict__ od_ptr1,
+                                                              const int64_t *__restrict__ od_pos1, const int32_t *__restrict__ od_col1,
+                                                              const double *__restrict__ vals, const int b, const int32_t *__restrict__ lev,
+                                                              const int32_t *__restrict__ off, const int *__restrict__ lev_ne,
+                                                              const long long *__restrict__ lev_off, double *__restrict__ ell,
+                                                              int32_t *__restrict__ ell_col, const int64_t n_brows) {
+    const int64_t pn = blockIdx.x;
+    const int side = blockIdx.y;
+    const int k = lev[pn];
+    const int ne = lev_ne[2 * k + side];
+    const int64_t *optr = side ? od_ptr1 : od_ptr0, *opos = side ? od_pos1 : od_pos0;
+    const int32_t *ocol = side ? od_col1 : od_col0;
+    const int64_t u0 = optr[pn], cnt = optr[pn + 1] - u0;
+    int32_t *cdst = ell_col + ((size_t)side * n_brows + pn) * DS_MAXNE;
+    for (int i = threadIdx.x; i < DS_MAXNE; i += blockDim.x) cdst[i] = i < cnt ? ocol[u0 + i] : -1;
+    if (ne == 0) return;
+    double *dst = ell + lev_off[2 * k + side] + (size_t)(pn - off[k]) * b * ne * b;   // [r][i][c]
+    for (int e = threadIdx.x; e < b * ne * b; e += blockDim.x) {
+        const int r = e / (ne * b), rem = e - r * ne * b, i = rem / b, c = rem - i * b;
+        dst[e] = i < cnt ? vals[((size_t)opos[u0 + i] * b + r) * b + c] : 0.0;
+    }
+}
+
+__device__ __forceinline__ uint32_t ds_smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void ds_mbar_init(uint64_t *bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(ds_smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void ds_mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(ds_smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void ds_mbar_arrive(uint64_t *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(ds_smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ bool ds_mbar_try(uint64_t *bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(ok)
+        : "r"(ds_smem_u32(bar)), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void ds_bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar, uint64_t policy) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+            ds_smem_u32(dst)),
+        "l"(src), "r"(bytes), "r"(ds_smem_u32(bar)), "l"(policy)
+        : "memory");
+}
+__device__ __forceinline__ void ds_prefetch_l2(const void *src, uint32_t bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ unsigned ds_ld_acquire(const unsigned *p) {
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+// Barrier over the consumer threads of all CTAs of the (co-resident) grid; the producer warps do not take part.
+__device__ __forceinline__ void ds_grid_barrier(unsigned *ctr, unsigned &target, const unsigned nctas) {
+    asm volatile("bar.sync 1, %0;" ::"n"(DS_WARPS * 32) : "memory");
+    if (threadIdx.x == 0) {
+        target += nctas;
+        __threadfence();   // cumulative: orders the writes of the whole CTA (made visible to this thread by bar.sync) before the arrival
+        atomicAdd(ctr, 1u);
+        while (ds_ld_acquire(ctr) < target) {
+        }
+        __threadfence();
+    }
+    asm volatile("bar.sync 1, %0;" ::"n"(DS_WARPS * 32) : "memory");
+}
+
+// The stream of one step for one CTA: first the packed off-diagonal rows [ra, rb) of (level k, side), `rps` rows per stage,
+// then the rows [ra, rb) of S_k^-1 in segments of DS_SEG doubles.
+struct DsStep {
+    const double *S, *ell;
+    int n, ra, rb, nseg, rowlen, rps, nA, nB;   // rowlen = ne * b doubles per packed row; nA / nB stages
+};
+__device__ __forceinline__ DsStep ds_step(const DirectSolveArgs &a, const int s, const int c, const int G) {
+    const int nsteps = 2 * a.nlev - 1;
+    const bool fwd = s < a.nlev;
+    const int k = fwd ? s : nsteps - 1 - s;
+    const DirectLevel L = a.lv[k];
+    DsStep d;
+    d.S = L.S;
+    d.n = L.n;
+    d.ra = (int)((long long)L.n * c / G);
+    d.rb = (int)((long long)L.n * (c + 1) / G);
+    d.nseg = (L.n + DS_SEG - 1) / DS_SEG;
+    const int ne = fwd ? L.ne[0] : L.ne[1];
+    d.rowlen = ne * a.b;
+    d.rps = d.rowlen > 0 ? DS_SEG / d.rowlen : 1;
+    d.ell = a.ell + (fwd ? L.ell_off[0] : L.ell_off[1]);
+    d.nA = d.rowlen > 0 ? (d.rb - d.ra + d.rps - 1) / d.rps : 0;
+    d.nB = (d.rb - d.ra) * d.nseg;
+    return d;
+}
+// source address and length (doubles) of stage i of a step's stream
+__device__ __forceinline__ const double *ds_stage_src(const DsStep &d, const int i, int &len) {
+    if (i < d.nA) {
+        const int r0 = d.ra + i * d.rps;
+        len = min(d.rps, d.rb - r0) * d.rowlen;
+        return d.ell + (size_t)r0 * d.rowlen;
+    }
+    const int j = i - d.nA;
+    const int row = d.ra + j / d.nseg, sg = j - (j / d.nseg) * d.nseg;
+    len = min(DS_SEG, d.n - sg * DS_SEG);
+    return d.S + (size_t)row * d.n + (size_t)sg * DS_SEG;
+}
+
+// column list (first DS_NCOL entries) and permutation entry of NEW block row `pn`: static data
+__device__ __forceinline__ void ds_load_cols(const DirectSolveArgs &a, const int side, const int pn, const bool have, int (&ncol)[DS_NCOL],
+                                             int &nperm) {
+    const int32_t *cl = a.ell_col + ((size_t)side * a.n_brows + pn) * DS_MAXNE;
+#pragma unroll
+    for (int w = 0; w < DS_NCOL; ++w) ncol[w] = have ? __ldg(cl + w) : -1;
+    nperm = have ? __ldg(a.perm + pn) : 0;
+}
+
+#ifdef MG_DS_STAMP   // development probe (compiled out in the library): per-phase global-timer stamps of CTA 0
+__device__ unsigned long long ds_stamps[16384];
+#define DS_STAMP(slot) \
+    if (blockIdx.x == 0 && (threadIdx.x & 31) == 0 && (threadIdx.x == 0 || threadIdx.x == DS_WARPS * 32) && s < 2000) { \
+        unsigned long long t__; \
+        asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t__)); \
+        ds_stamps[s * 8 + (slot)] = t__; \
+    }
+#else
+#define DS_STAMP(slot)
+#endif
+
+__global__ void __launch_bounds__(DS_THREADS, 1) direct_solve_persistent_kernel(const DirectSolveArgs a) {
+    extern __shared__ __align__(128) unsigned char ds_smem[];
+    double *ring = reinterpret_cast<double *>(ds_smem);
+    double *tsm = ring + (size_t)a.stages * DS_SEG;
+    uint64_t *full = reinterpret_cast<uint64_t *>(tsm + a.tcap);
+    uint64_t *empty = full + a.stages;
+    volatile int *round_of = reinterpret_cast<volatile int *>(empty + a.stages);   // rounds for which a stage has been issued
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int G = gridDim.x, c = blockIdx.x, b = a.b, ST = a.stages;
+    if (tid == 0) {
+        for (int s = 0; s < ST; ++s) {
+            round_of[s] = 0;
+            ds_mbar_init(&full[s], 1);
+            ds_mbar_init(&empty[s], 1);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    const int nsteps = 2 * a.nlev - 1;
+
+    if (warp == DS_WARPS) {
+        // ---------------------------------------------------------------- producer: the CTA's static matrix stream
+        uint64_t pol;
+        asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+        long long cnt = 0;
+        // L2 prefetch cursor: runs DS_LOOKAHEAD stages ahead of the issue cursor, across step boundaries
+        long long pabs = 0;            // absolute index of the next stage to prefetch
+        int pstep = 0, pidx = 0;
+        DsStep dp = ds_step(a, 0, c, G);
+        for (int s = 0; s < nsteps; ++s) {
+            const DsStep d = ds_step(a, s, c, G);
+            const int total = d.nA + d.nB;
+            for (int base = 0; base < total; base += DS_PL) {
+                const long long want = cnt + base + DS_PL + DS_LOOKAHEAD;
+                while (pabs < want && pstep < nsteps) {
+                    const int ptotal = dp.nA + dp.nB;
+                    const int take = (int)min((long long)min(32, ptotal - pidx), want - pabs);
+                    if (take <= 0) {
+                        if (++pstep < nsteps) dp = ds_step(a, pstep, c, G);
+                        pidx = 0;
+                        continue;
+                    }
+                    if (lane < take && pabs + lane >= cnt + base + DS_PL) {   // (stages about to be issued are not worth a prefetch)
+                        int len;
+                        const double *src = ds_stage_src(dp, pidx + lane, len);
+                        ds_prefetch_l2(src, (uint32_t)(len * sizeof(double)));
+                    }
+                    pidx += take;
+                    pabs += take;
+                }
+                const int i = base + lane;
+                if (lane < DS_PL && i < total) {
+                    const long long cc = cnt + i;
+                    const int st = (int)(cc % ST);
+                    const int round = (int)(cc / ST);
+                    while (!ds_mbar_try(&empty[st], ((uint32_t)round & 1u) ^ 1u)) {
+                    }
+                    round_of[st] = round + 1;
+                    int len;
+                    const double *src = ds_stage_src(d, i, len);
+                    ds_mbar_expect_tx(&full[st], (uint32_t)(len * sizeof(double)));
+                    ds_bulk_g2s(ring + (size_t)st * DS_SEG, src, (uint32_t)(len * sizeof(double)), &full[st], pol);
+                }
+                __syncwarp();
+            }
+            cnt += total;
+            DS_STAMP(7);
+        }
+        return;
+    }
+
+    // -------------------------------------------------------------------- consumers
+    unsigned bar_target = 0;
+    long long cnt = 0;
+    int ncol[DS_NCOL], nperm = 0;   // column list / permutation entry of this thread's row in the coming step (first pass)
+    {
+        const DsStep d0 = ds_step(a, 0, c, G);
+        const int q = tid / DS_TPR;
+        ds_load_cols(a, 0, a.lv[0].first + (d0.ra + (q < d0.rb - d0.ra ? q : 0)) / b, q < d0.rb - d0.ra, ncol, nperm);
+    }
+    for (int s = 0; s < nsteps; ++s) {
+        const bool fwd = s < a.nlev;
+        const int k = fwd ? s : nsteps - 1 - s;
+        const DsStep d = ds_step(a, s, c, G);
+        const int first = a.lv[k].first;
+        DS_STAMP(0);
+        // ---- (A) t = z_k - L_k y_{k-1}   or   t = U_k x_{k+1}   for the rows [ra, rb): DS_TPR threads per scalar row, packed
+        // block rows out of the ring; the column lists (static) were fetched before the preceding grid barrier, so the
+        // gathered y / x values are the only global round trip here, all of a thread's loads in flight at once
+        {
+            const int nr = d.rb - d.ra;
+            constexpr int RPP = DS_WARPS * 32 / DS_TPR;   // rows per pass
+            for (int q0 = 0; q0 < nr; q0 += RPP) {
+                const int q = q0 + tid / DS_TPR, sub = tid % DS_TPR;
+                const bool have = q < nr;
+                const int row = d.ra + (have ? q : 0), pl = row / b, r = row - pl * b;
+                if (q0 != 0) ds_load_cols(a, fwd ? 0 : 1, first + pl, have, ncol, nperm);
+                double acc = 0.0;
+                double zv = 0.0;
+                if (have && fwd) zv = __ldg(a.rhs + (size_t)nperm * b + r);
+                if (have && d.rowlen > 0) {
+                    const long long cc = cnt + q / d.rps;
+                    const int st = (int)(cc % ST);
+                    const int round = (int)(cc / ST);
+                    while (round_of[st] <= round) __nanosleep(100);
+                    while (!ds_mbar_try(&full[st], (uint32_t)round & 1u)) {
+                    }
+                    const double *As = ring + (size_t)st * DS_SEG + (size_t)(q - (q / d.rps) * d.rps) * d.rowlen;
+                    for (int f0 = sub; f0 < d.rowlen; f0 += DS_TPR * DS_XCH) {
+                        double xv[DS_XCH];
+#pragma unroll
+                        for (int u = 0; u < DS_XCH; ++u) {
+                            const int f = f0 + u * DS_TPR;
+                            xv[u] = 0.0;
+                            if (f < d.rowlen) {
+                                const int ie = f / b, cx = f - ie * b;
+                                int col = -1;
+#pragma unroll
+                                for (int w = 0; w < DS_NCOL; ++w) col = (ie == w) ? ncol[w] : col;
+                                if (ie >= DS_NCOL) col = __ldg(a.ell_col + ((size_t)(fwd ? 0 : 1) * a.n_brows + first + pl) * DS_MAXNE + ie);
+                                if (col >= 0) xv[u] = __ldcg(a.yb + (size_t)col * b + cx);
+                            }
+                        }
+#pragma unroll
+                        for (int u = 0; u < DS_XCH; ++u) {
+                            const int f = f0 + u * DS_TPR;
+                            if (f < d.rowlen) acc = fma(As[f], xv[u], acc);
+                        }
+                    }
+                }
+#pragma unroll
+                for (int o = DS_TPR / 2; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+                if (have && sub == 0) a.tb[row] = fwd ? zv - acc : acc;
+            }
+        }
+        // all rows of the step's packed stages are consumed once every consumer warp is here: hand the stages back
+        asm volatile("bar.sync 1, %0;" ::"n"(DS_WARPS * 32) : "memory");
+        for (int i = tid; i < d.nA; i += DS_WARPS * 32) ds_mbar_arrive(&empty[(int)((cnt + i) % ST)]);
+        cnt += d.nA;
+        DS_STAMP(1);
+        ds_grid_barrier(a.bar, bar_target, (unsigned)G);
+        DS_STAMP(2);
+        // ---- (B) rows of S_k^-1 times t
+        for (int i0 = 0; i0 < d.n; i0 += 8 * 2 * DS_WARPS * 32) {   // 8 independent 128-bit loads in flight per thread (n even)
+            double2 tv[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const int i = i0 + 2 * (tid + u * DS_WARPS * 32);
+                tv[u] = i < d.n ? __ldcg(reinterpret_cast<const double2 *>(a.tb + i)) : make_double2(0.0, 0.0);
+            }
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const int i = i0 + 2 * (tid + u * DS_WARPS * 32);
+                if (i < d.n) *reinterpret_cast<double2 *>(tsm + i) = tv[u];
+            }
+        }
+        asm volatile("bar.sync 1, %0;" ::"n"(DS_WARPS * 32) : "memory");
+        DS_STAMP(3);
+        for (int i = warp; i < d.rb - d.ra; i += DS_WARPS) {
+            const int row = d.ra + i;
+            double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+            for (int sg = 0; sg < d.nseg; ++sg) {
+                const long long cc = cnt + (long long)i * d.nseg + sg;
+                const int st = (int)(cc % ST);
+                const int round = (int)(cc / ST);
+                while (round_of[st] <= round) __nanosleep(100);
+                while (!ds_mbar_try(&full[st], (uint32_t)round & 1u)) {
+                }
+                const int len2 = min(DS_SEG, d.n - sg * DS_SEG) >> 1;
+                const double2 *A2 = reinterpret_cast<const double2 *>(ring + (size_t)st * DS_SEG);
+                const double2 *t2 = reinterpret_cast<const double2 *>(tsm + (size_t)sg * DS_SEG);
+                int e = lane;
+                for (; e + 32 < len2; e += 64) {
+                    const double2 v0 = A2[e], v1 = A2[e + 32];
+                    const double2 y0 = t2[e], y1 = t2[e + 32];
+                    s0 = fma(v0.x, y0.x, s0);
+                    s1 = fma(v0.y, y0.y, s1);
+                    s2 = fma(v1.x, y1.x, s2);
+                    s3 = fma(v1.y, y1.y, s3);
+                }
+                if (e < len2) {
+                    const double2 v0 = A2[e], y0 = t2[e];
+                    s0 = fma(v0.x, y0.x, s0);
+                    s1 = fma(v0.y, y0.y, s1);
+                }
+                __syncwarp();
+                if (lane == 0) ds_mbar_arrive(&empty[st]);
+            }
+            double sum = (s0 + s1) + (s2 + s3);
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+            if (lane == 0) {
+                const size_t gi = (size_t)first * b + row;
+                const double yv = fwd ? sum : __ldcg(a.yb + gi) - sum;
+                a.yb[gi] = yv;
+                if (!fwd || k == a.nlev - 1) {   // final value of this row: scatter to the natural ordering
+                    const int pl = row / b;
+                    a.e[(size_t)__ldg(a.perm + first + pl) * b + (row - pl * b)] = yv;
+                }
+            }
+        }
+        cnt += d.nB;
+        DS_STAMP(4);
+        if (s + 1 < nsteps) {   // static data of the coming step's first pass, fetched behind the grid barrier
+            const DsStep dn = ds_step(a, s + 1, c, G);
+            const bool fn = s + 1 < a.nlev;
+            const int kn = fn ? s + 1 : nsteps - 2 - s;
+            const int q = tid / DS_TPR;
+            ds_load_cols(a, fn ? 0 : 1, a.lv[kn].first + (dn.ra + (q < dn.rb - dn.ra ? q : 0)) / b, q < dn.rb - dn.ra, ncol, nperm);
+        }
+        DS_STAMP(5);
+        ds_grid_barrier(a.bar, bar_target, (unsigned)G);
+        DS_STAMP(6);
+    }
 }
 
 }  // namespace mgk

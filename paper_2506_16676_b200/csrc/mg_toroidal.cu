@@ -91,6 +91,19 @@ struct DirectCoarse {
     int *bad = nullptr;
     int maxn = 0;
     int64_t bytes = 0;
+    // persistent cooperative solve kernel (direct_solve_persistent_kernel); the launch chain is the fallback
+    bool persist = false;
+    DirectLevel *lvdev = nullptr;
+    unsigned *bar = nullptr;
+    int ds_grid = 0, ds_stages = 0, ds_tcap = 0;
+    size_t ds_smem = 0;
+    std::vector<int32_t> first;   // first new block position of every level set
+    int64_t offdiag_blocks = 0;   // stored blocks of all L_k and U_k
+    double *ell = nullptr;        // packed (ELL) off-diagonal block rows in the level-set ordering, both sides
+    int32_t *ell_col = nullptr;   // [2][n_brows][DS_MAXNE]
+    int *lev_ne = nullptr;        // device [nlev][2]
+    long long *lev_off = nullptr; // device [nlev][2]
+    int64_t ell_doubles = 0;
 };
 
 }  // namespace
@@ -100,6 +113,7 @@ struct mg_handle {
     int b = 0, n_pol = 0, n_phi = 0, n_levels = 0;
     int sm_count = 148;
     bool coop_ok = false;    // cooperative launches available and gmres_orth_fused_kernel's shared memory opted in
+    bool coop_launch = false;  // the device supports cooperative launches
     double *frag_part = nullptr;  // TMA kernel: partial sums of rows that straddle two CTAs (sm_count x 36)
     int *frag_flag = nullptr;
     bool tma_ready = false;  // b == 36 and the kernel's shared-memory attribute is set
@@ -107,6 +121,7 @@ struct mg_handle {
     cudaStream_t cap_stream = nullptr;  // internal non-default stream (the legacy default stream cannot capture)
     std::vector<Level> lev;
     std::vector<void *> owned;
+    std::vector<size_t> owned_bytes;   // parallel to `owned`
     int64_t dev_bytes = 0;
     int64_t launches = 0;
     int *pinned = nullptr;        // 8 ints + 4 doubles of pinned host scratch
@@ -263,6 +278,7 @@ int dalloc(mg_handle *h, void **p, size_t bytes) {
         }
     }
     h->owned.push_back(q);
+    h->owned_bytes.push_back(bytes);
     h->dev_bytes += (int64_t)bytes;
     *p = q;
     return MG_OK;
@@ -270,6 +286,21 @@ int dalloc(mg_handle *h, void **p, size_t bytes) {
 template <typename T>
 int dalloc_t(mg_handle *h, T **p, size_t count) {
     return dalloc(h, reinterpret_cast<void **>(p), count * sizeof(T));
+}
+// Release one allocation of the handle before mg_destroy (buffers that are re-sized: the Krylov bases).
+template <typename T>
+void dfree_t(mg_handle *h, T *&p) {
+    if (p == nullptr) return;
+    auto it = std::find(h->owned.begin(), h->owned.end(), static_cast<void *>(p));
+    if (it != h->owned.end()) {
+        const size_t idx = (size_t)(it - h->owned.begin());
+        h->dev_bytes -= (int64_t)h->owned_bytes[idx];
+        h->owned_bytes.erase(h->owned_bytes.begin() + idx);
+        h->owned.erase(it);
+        if (h->opt.free) h->opt.free(p, h->opt.alloc_ctx);
+        else if (!h->opt.alloc) cudaFree(p);
+    }
+    p = nullptr;
 }
 
 inline int grid_for(int64_t n, int per_block, int cap = 148 * 16) {
@@ -457,7 +488,43 @@ int prolong_add(mg_handle *h, int l, const double *ec, double *xf, double *pe) {
 }
 
 // ------------------------------------------------------------------------------------------------ GMRES engine
+// Frees the buffers of a previous gmres_alloc (restart length or iteration cap changed): without this every change of
+// `restart` / `maxit` leaked a whole Krylov basis until mg_destroy.
+void gmres_release(mg_handle *h, Gmres &G) {
+    if (!G.ready) return;
+    cudaStreamSynchronize(h->stream);   // kernels in flight may still use the old buffers
+    dfree_t(h, G.V);
+    dfree_t(h, G.Z);
+    dfree_t(h, G.partial);
+    dfree_t(h, G.counter);
+    GmresDev &d = G.dev;
+    dfree_t(h, d.H);
+    dfree_t(h, d.cs);
+    dfree_t(h, d.sn);
+    dfree_t(h, d.g);
+    dfree_t(h, d.y);
+    dfree_t(h, d.h1);
+    dfree_t(h, d.h2);
+    dfree_t(h, d.nrm2);
+    dfree_t(h, d.hnext);
+    dfree_t(h, d.tol);
+    dfree_t(h, d.hist);
+    dfree_t(h, d.status);
+    dfree_t(h, G.orth_partial);
+    dfree_t(h, G.orth_nrm);
+    dfree_t(h, G.orth_counter);
+    G.ready = false;
+}
+
 int gmres_alloc(mg_handle *h, Gmres &G, int64_t n, int m, int maxit, bool flexible) {
+    if (G.ready && G.n == n && G.m == m && G.flexible == flexible) {   // only the iteration cap changed: the history buffer
+        dfree_t(h, G.dev.hist);
+        G.maxit = maxit;
+        G.dev.maxit = maxit;
+        MG(dalloc_t(h, &G.dev.hist, (size_t)maxit + 2));
+        return MG_OK;
+    }
+    gmres_release(h, G);
     G.n = n;
     G.m = m;
     G.maxit = maxit;
@@ -747,6 +814,7 @@ int direct_symbolic(mg_handle *h) {
     // row-wise lists of the off-diagonal blocks for the solve: side 0 = L (column one level set down), 1 = U (one up)
     std::vector<int64_t> od_ptr[2], od_pos[2];
     std::vector<int32_t> od_col[2];
+    dc.offdiag_blocks = 0;
     for (int side = 0; side < 2; ++side) {
         const int want = side == 0 ? -1 : 1;
         od_ptr[side].assign((size_t)n + 1, 0);
@@ -760,6 +828,7 @@ int direct_symbolic(mg_handle *h) {
             }
             od_ptr[side][pn + 1] = (int64_t)od_pos[side].size();
         }
+        dc.offdiag_blocks += (int64_t)od_pos[side].size();
         if (od_pos[side].empty()) {
             od_pos[side].push_back(0);
             od_col[side].push_back(0);
@@ -820,6 +889,77 @@ int direct_symbolic(mg_handle *h) {
         MG(dalloc_t(h, &dc.rob, (size_t)std::max<int64_t>(L.nnzb, 1)));
         LAUNCH(h, rows_of_blocks_kernel, grid_for(n, 256, 1 << 30), 256, 0, L.row_ptr, n, dc.rob);
     }
+    // persistent solve kernel: needs 16-byte aligned rows (b even), b <= 64, ELL width <= DS_MAXNE, t and >= DS_PL ring stages
+    // in shared memory, and the packed stages of one step of one CTA must fit the ring together
+    dc.first.assign(off.begin(), off.end());
+    dc.persist = false;
+    {
+        std::vector<int> lev_ne((size_t)2 * dc.nlev, 0);
+        std::vector<long long> lev_off((size_t)2 * dc.nlev, 0);
+        int ne_max = 0;
+        for (int side = 0; side < 2; ++side)
+            for (int64_t pn = 0; pn < n; ++pn) {
+                const int cnt = (int)(od_ptr[side][pn + 1] - od_ptr[side][pn]);
+                int &m = lev_ne[2 * lev_new[pn] + side];
+                m = std::max(m, cnt);
+                ne_max = std::max(ne_max, cnt);
+            }
+        long long ell_doubles = 0;
+        for (int k = 0; k < dc.nlev; ++k)
+            for (int side = 0; side < 2; ++side) {
+                lev_off[2 * k + side] = ell_doubles;
+                ell_doubles += (long long)dc.nk[k] * lev_ne[2 * k + side] * b;
+            }
+        const int tcap = (dc.maxn + 1) / 2 * 2;
+        const size_t budget = 227 * 1024;
+        int stages = 0;
+        if (direct_smem_bytes(DS_PL, tcap) <= budget)
+            stages = (int)std::min<size_t>(64, (budget - direct_smem_bytes(0, tcap)) / (sizeof(double) * DS_SEG + 2 * sizeof(uint64_t) + sizeof(int)));
+        bool fits = (b % 2 == 0) && b <= 64 && ne_max <= DS_MAXNE && stages >= DS_PL && h->coop_launch;
+        for (int k = 0; fits && k < dc.nlev; ++k)
+            for (int side = 0; side < 2; ++side) {
+                const int rowlen = lev_ne[2 * k + side] * b;
+                if (rowlen == 0) continue;
+                const int rps = DS_SEG / rowlen, nr = dc.nk[k] / h->sm_count + 2;
+                if (rps < 1 || (nr + rps - 1) / rps > stages - 1) fits = false;
+            }
+        int per_sm = 0;
+        if (fits &&
+            cudaFuncSetAttribute(direct_solve_persistent_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)direct_smem_bytes(stages, tcap)) == cudaSuccess &&
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, direct_solve_persistent_kernel, DS_THREADS,
+                                                          direct_smem_bytes(stages, tcap)) == cudaSuccess && per_sm >= 1) {
+            dc.ds_stages = stages;
+            dc.ds_tcap = tcap;
+            dc.ds_smem = direct_smem_bytes(stages, tcap);
+            dc.ds_grid = h->sm_count;
+            dc.ell_doubles = ell_doubles;
+            MG(dalloc_t(h, &dc.lvdev, (size_t)dc.nlev));
+            MG(dalloc_t(h, &dc.bar, 4));
+            MG(dalloc_t(h, &dc.ell, (size_t)std::max<long long>(ell_doubles, 2)));
+            MG(dalloc_t(h, &dc.ell_col, (size_t)2 * n * DS_MAXNE));
+            MG(dalloc_t(h, &dc.lev_ne, (size_t)2 * dc.nlev));
+            MG(dalloc_t(h, &dc.lev_off, (size_t)2 * dc.nlev));
+            std::vector<DirectLevel> lv((size_t)dc.nlev);
+            for (int k = 0; k < dc.nlev; ++k) {
+                lv[k].S = dc.S[k];
+                lv[k].n = dc.nk[k];
+                lv[k].first = off[k];
+                for (int side = 0; side < 2; ++side) {
+                    lv[k].ell_off[side] = lev_off[2 * k + side];
+                    lv[k].ne[side] = lev_ne[2 * k + side];
+                }
+            }
+            CU(cudaMemcpyAsync(dc.lvdev, lv.data(), sizeof(DirectLevel) * dc.nlev, cudaMemcpyHostToDevice, h->stream));
+            CU(cudaMemcpyAsync(dc.lev_ne, lev_ne.data(), sizeof(int) * 2 * dc.nlev, cudaMemcpyHostToDevice, h->stream));
+            CU(cudaMemcpyAsync(dc.lev_off, lev_off.data(), sizeof(long long) * 2 * dc.nlev, cudaMemcpyHostToDevice, h->stream));
+            CU(cudaMemsetAsync(dc.yb, 0, sizeof(double) * ((size_t)L.nvec + 2), h->stream));
+            CU(cudaStreamSynchronize(h->stream));
+            dc.persist = true;
+        } else {
+            cudaGetLastError();
+        }
+    }
     CU(cudaStreamSynchronize(h->stream));   // the host vectors above are locals
     dc.symbolic = true;
     return MG_OK;
@@ -836,6 +976,8 @@ int dense_inverse_inplace(mg_handle *h, double *A, int n) {
     CU(cudaGetLastError());
     return MG_OK;
 }
+
+int direct_solve(mg_handle *h, const double *rhs, double *e);
 
 // Numeric part (setup and every refresh): assemble the dense diagonal blocks, then S_k = D_k - (L_k S_{k-1}^-1) U_{k-1}
 // and its inverse, level set by level set.
@@ -860,11 +1002,32 @@ int direct_numeric(mg_handle *h) {
         }
         MG(dense_inverse_inplace(h, dc.S[k], dc.nk[k]));
     }
+    if (dc.persist) {   // off-diagonal block rows in the level-set ordering, one contiguous span per level set and side
+        LAUNCH(h, direct_pack_ell_kernel, dim3((unsigned)L.n_brows, 2), 128, 0, dc.od_ptr[0], dc.od_pos[0], dc.od_col[0], dc.od_ptr[1],
+               dc.od_pos[1], dc.od_col[1], L.vals, b, dc.lev, dc.off, dc.lev_ne, dc.lev_off, dc.ell, dc.ell_col, L.n_brows);
+        CU(cudaGetLastError());
+    }
     int bad = 0;
     CU(cudaMemcpyAsync(&bad, dc.bad, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
     CU(cudaStreamSynchronize(h->stream));
     if (bad == 2) return MG_ESINGULAR;
     dc.numeric = true;
+    // The Schur complements are inverted WITHOUT pivoting (fine for operators with a positive definite symmetric part, which
+    // the Galerkin hierarchy of the paper's elliptic systems has): one probe solve checks the factorisation, so that a small
+    // pivot on some other operator is an error code and not a silently inaccurate coarse solve.
+    {
+        LAUNCH(h, hashed_start_kernel, grid_for(L.nvec, 256), 256, 0, L.d[0], L.nvec);
+        const int rc = direct_solve(h, L.d[0], L.d[1]);
+        if (rc != MG_OK) { dc.numeric = false; return rc; }
+        MG(residual(h, L, L.d[0], L.d[1], L.pe));
+        double rr = 0.0, bb = 0.0;
+        MG(dot_host(h, L.pe, L.pe, L.nvec, &rr));
+        MG(dot_host(h, L.d[0], L.d[0], L.nvec, &bb));
+        if (!(rr <= 1e-12 * bb)) {   // relative residual above 1e-6 (or NaN)
+            dc.numeric = false;
+            return MG_ESINGULAR;
+        }
+    }
     return MG_OK;
 }
 
@@ -873,8 +1036,34 @@ int direct_numeric(mg_handle *h) {
 int direct_solve(mg_handle *h, const double *rhs, double *e) {
     Level &L = h->lev.back();
     DirectCoarse &dc = h->direct;
-    KindScope scope(h, L.index, MG_KIND_OTHER);
+    KindScope scope(h, L.index, MG_KIND_DIRECT);
     const int b = h->b;
+    if (dc.persist && h->opt.kernel_variant == 0) {
+        DirectSolveArgs a{};
+        a.lv = dc.lvdev;
+        a.nlev = dc.nlev;
+        a.b = b;
+        a.ell = dc.ell;
+        a.ell_col = dc.ell_col;
+        a.n_brows = L.n_brows;
+        a.perm = dc.perm;
+        a.rhs = rhs;
+        a.e = e;
+        a.yb = dc.yb;
+        a.tb = dc.tb;
+        a.bar = dc.bar;
+        a.stages = dc.ds_stages;
+        a.tcap = dc.ds_tcap;
+        CU(cudaMemsetAsync(dc.bar, 0, sizeof(unsigned), h->stream));
+        void *params[] = {&a};
+        ProfPair pp;
+        const bool prof = prof_begin(h, pp);
+        CU(cudaLaunchCooperativeKernel((const void *)direct_solve_persistent_kernel, dim3(dc.ds_grid), dim3(DS_THREADS), params,
+                                       dc.ds_smem, h->stream));
+        if (prof) prof_end(h, pp);
+        count_launch(h);
+        return MG_OK;
+    }
     LAUNCH_PDL(h, permute_blocks_kernel, grid_for(L.nvec, 256, 1 << 30), 256, 0, rhs, dc.zb, dc.perm, L.n_brows, b, 0);
     for (int k = 0; k < dc.nlev; ++k) {   // y_k = S_k^-1 (z_k - L_k y_{k-1})
         const double *zk = dc.zb + dc.voff[k];
@@ -1238,6 +1427,9 @@ int build_coarse_level(mg_handle *h, int l) {
 }
 
 bool level_ok(mg_handle *h, int level) { return h && level >= 0 && level < h->n_levels; }
+// Vectors and matrix arrays must be 16-byte aligned: the TMA kernels issue bulk copies from them (a misaligned pointer
+// would be a device fault, not an error code).
+inline bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 }  // namespace
 
@@ -1308,7 +1500,7 @@ int mg_setup(mg_handle **out, const int64_t *row_ptr, const int32_t *col_idx, co
              int n_phi, int levels, const mg_options *opt, void *cuda_stream) {
     if (!out) return MG_EINVAL;
     *out = nullptr;
-    if (!row_ptr || !col_idx || !vals) return MG_EINVAL;
+    if (!row_ptr || !col_idx || !vals || !aligned16(vals)) return MG_EINVAL;
     if (b < 1 || b > 64 || n_pol < 1 || n_phi < 1 || levels < 1 || levels > 30) return MG_EINVAL;
     if (n_phi % (1 << (levels - 1)) != 0) return MG_EINVAL;
     mg_options o;
@@ -1347,7 +1539,8 @@ int mg_setup(mg_handle **out, const int64_t *row_ptr, const int32_t *col_idx, co
         if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
             h->sm_count = sms;
         int coop = 0;
-        if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) == cudaSuccess && coop &&
+        if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) == cudaSuccess && coop) h->coop_launch = true;
+        if (h->coop_launch &&
             cudaFuncSetAttribute(gmres_orth_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024) == cudaSuccess)
             h->coop_ok = true;
         else
@@ -1410,6 +1603,12 @@ int mg_update_options(mg_handle *h, const mg_options *opt) {
 
 int mg_update_values(mg_handle *h, const double *vals) {
     if (!h || !vals) return MG_EINVAL;
+    if (!aligned16(vals)) return MG_EINVAL;
+    if (h->coarse_graph && h->n_levels == 1) {   // the captured coarse cycle holds level 0's old (borrowed) values pointer
+        cudaStreamSynchronize(h->stream);
+        cudaGraphExecDestroy(h->coarse_graph);
+        h->coarse_graph = nullptr;
+    }
     h->lev[0].vals = vals;
     h->outer_vals = nullptr;
     for (int l = 0; l < h->n_levels; ++l) {
@@ -1426,18 +1625,18 @@ int mg_update_values(mg_handle *h, const double *vals) {
 }
 
 int mg_set_operator(mg_handle *h, const double *vals) {
-    if (!h) return MG_EINVAL;
+    if (!h || !aligned16(vals)) return MG_EINVAL;
     h->outer_vals = vals;
     return MG_OK;
 }
 
 int mg_vcycle(mg_handle *h, const double *r, double *z) {
-    if (!h || !r || !z || r == z) return MG_EINVAL;
+    if (!h || !r || !z || r == z || !aligned16(r) || !aligned16(z)) return MG_EINVAL;
     return vcycle_internal(h, r, z);
 }
 
 int mg_solve(mg_handle *h, const double *rhs, double *x, double rtol, int x_is_initial_guess, mg_solve_info *info) {
-    if (!h || !rhs || !x || rhs == x || !(rtol > 0.0)) return MG_EINVAL;
+    if (!h || !rhs || !x || rhs == x || !(rtol > 0.0) || !aligned16(rhs) || !aligned16(x)) return MG_EINVAL;
     Level L = h->lev[0];  // the operator of the Krylov iteration: level 0's pattern with the current operator values
     L.h_row_ptr.clear();
     L.h_col_idx.clear();
@@ -1532,22 +1731,22 @@ int mg_solve_host(mg_handle *h, const double *rhs_host, double *x_host, double r
 }
 
 int mg_spmv(mg_handle *h, int level, const double *x, double *y) {
-    if (!level_ok(h, level) || !x || !y || x == y) return MG_EINVAL;
+    if (!level_ok(h, level) || !x || !y || x == y || !aligned16(x) || !aligned16(y)) return MG_EINVAL;
     return spmv(h, h->lev[level], x, y);
 }
 
 int mg_residual(mg_handle *h, int level, const double *rhs, const double *x, double *r) {
-    if (!level_ok(h, level) || !rhs || !x || !r || x == r) return MG_EINVAL;
+    if (!level_ok(h, level) || !rhs || !x || !r || x == r || !aligned16(rhs) || !aligned16(x) || !aligned16(r)) return MG_EINVAL;
     return residual(h, h->lev[level], rhs, x, r);
 }
 
 int mg_pbj_apply(mg_handle *h, int level, const double *r, double *z) {
-    if (!level_ok(h, level) || !r || !z) return MG_EINVAL;
+    if (!level_ok(h, level) || !r || !z || !aligned16(r) || !aligned16(z)) return MG_EINVAL;
     return pbj(h, h->lev[level], r, z, 1.0);
 }
 
 int mg_smooth(mg_handle *h, int level, const double *rhs, double *x, int nu, int zero_guess) {
-    if (!level_ok(h, level) || !rhs || !x || nu < 0 || rhs == x) return MG_EINVAL;
+    if (!level_ok(h, level) || !rhs || !x || nu < 0 || rhs == x || !aligned16(rhs) || !aligned16(x)) return MG_EINVAL;
     Level &L = h->lev[level];
     if (h->opt.smoother == 1) return gmres_smooth(h, L, rhs, x, nu, zero_guess != 0);
     if (zero_guess) return presmooth(h, L, rhs, x, nu);
@@ -1569,7 +1768,7 @@ int mg_prolong_add(mg_handle *h, int level, const double *e_coarse, double *x_fi
 }
 
 int mg_coarse_solve(mg_handle *h, const double *r, double *e, int *iters) {
-    if (!h || !r || !e) return MG_EINVAL;
+    if (!h || !r || !e || !aligned16(r) || !aligned16(e)) return MG_EINVAL;
     Level &L = h->lev.back();
     const size_t bytes = (size_t)L.nvec * sizeof(double);
     CU(cudaMemcpyAsync(L.rhs, r, bytes, cudaMemcpyDeviceToDevice, h->stream));
@@ -1577,6 +1776,19 @@ int mg_coarse_solve(mg_handle *h, const double *r, double *e, int *iters) {
     CU(cudaMemcpyAsync(e, L.x, bytes, cudaMemcpyDeviceToDevice, h->stream));
     CU(cudaStreamSynchronize(h->stream));
     if (iters) *iters = h->coarse_iters_last;
+    return MG_OK;
+}
+
+int mg_direct_info(mg_handle *h, int *level_sets, int64_t *dense_bytes, int64_t *offdiag_bytes, int *max_n, int *persistent) {
+    if (!h || !h->direct.symbolic) return MG_EINVAL;
+    const DirectCoarse &dc = h->direct;
+    int64_t dense = 0;
+    for (int k = 0; k < dc.nlev; ++k) dense += (int64_t)sizeof(double) * dc.nk[k] * dc.nk[k];
+    if (level_sets) *level_sets = dc.nlev;
+    if (dense_bytes) *dense_bytes = dense;
+    if (offdiag_bytes) *offdiag_bytes = dc.offdiag_blocks * (int64_t)sizeof(double) * h->b * h->b;   // (the packed copy is padded)
+    if (max_n) *max_n = dc.maxn;
+    if (persistent) *persistent = (dc.persist && h->opt.kernel_variant == 0) ? 1 : 0;
     return MG_OK;
 }
 
@@ -1658,6 +1870,12 @@ const char *mg_strerror(int code) {
         default: return "unknown error code";
     }
 }
+
+#ifdef MG_DS_STAMP
+int mg_debug_ds_stamps(unsigned long long *host, int n) {
+    return cudaMemcpyFromSymbol(host, mgk::ds_stamps, sizeof(unsigned long long) * n) == cudaSuccess ? 0 : -1;
+}
+#endif
 
 const char *mg_version(void) { return "mg_toroidal 0.1.0 (sm_100a)"; }
 

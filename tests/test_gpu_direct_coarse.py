@@ -29,9 +29,10 @@ def make(case, **opt):
     return w, H, s
 
 
+@pytest.mark.parametrize("variant", [0, 1])   # 0: the persistent cooperative kernel (where its requirements hold), 1: the launch chain
 @pytest.mark.parametrize("case", list(CASES))
-def test_direct_coarse_solve_and_cycle(case):
-    w, H, s = make(case)
+def test_direct_coarse_solve_and_cycle(case, variant):
+    w, H, s = make(case, kernel_variant=variant)
     try:
         Lc = H.levels[-1]
         rc = input_vector(Lc.n, w.seed, 61)

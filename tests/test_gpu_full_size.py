@@ -108,3 +108,31 @@ def test_c1_default_mode_properties(c1):
         assert np.linalg.norm(rc - mg.spmv(Lc, to_np(e))) <= 1.01e-10 * np.linalg.norm(rc)
     finally:
         s.update_options(coarse_mode=1, maxit=400)
+
+
+def test_c1_direct_coarse_solve(c1):
+    """coarse_mode = 2 at full C1 size (4,000 block rows on the coarsest level, 60 level sets of ~2,900 scalars; the
+    persistent cooperative kernel with 148 CTAs): an exact solve on the ORACLE's coarsest matrix, and the complete solve
+    against the oracle's stored run (tests/golden/solve_C1_direct.json: sparse LU on the oracle's side)."""
+    import json
+    import os
+    w, H, s = c1
+    s.update_options(coarse_mode=2)
+    try:
+        Lc = H.levels[-1]
+        rc = input_vector(Lc.n, w.seed, 61)
+        e, it = s.coarse_solve(to_dev(rc))
+        assert it == 0
+        assert np.linalg.norm(rc - mg.spmv(Lc, to_np(e))) <= 1e-11 * np.linalg.norm(rc)
+        e2, _ = s.coarse_solve(to_dev(rc))
+        assert np.array_equal(to_np(e2), to_np(e))          # bit-reproducible from call to call
+        path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "solve_C1_direct.json")
+        if os.path.exists(path):
+            with open(path) as f:
+                g = json.load(f)
+            x, info = s.solve(to_dev(w.rhs), rtol=1e-8, hist_cap=512)
+            assert info["converged"] and abs(info["iters"] - g["iters"]) <= 1
+            k = min(len(g["hist"]), len(info["hist"]))
+            assert np.abs(np.log10(np.array(info["hist"][:k]) / np.array(g["hist"][:k]))).max() <= 0.05
+    finally:
+        s.update_options(coarse_mode=1)
