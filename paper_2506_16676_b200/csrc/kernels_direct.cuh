@@ -4,13 +4,19 @@
 // The block rows of the coarsest level are ordered by the level sets of a breadth-first search of its block graph: every
 // block then couples only rows of the same or of adjacent level sets, i.e. the matrix is BLOCK TRIDIAGONAL with dense
 // diagonal blocks D_k (n_k x n_k) and SPARSE off-diagonal blocks L_k (n_k x n_{k-1}), U_k (n_k x n_{k+1}), which stay in
-// the level's block-CSR storage.  Setup (off the solve path) forms the inverses of the Schur complements explicitly,
-//      S_0 = D_0,   S_k = D_k - (L_k S_{k-1}^-1) U_{k-1},
-// (only S_k^-1 is kept: sum_k n_k^2 doubles plus one n_k x n_{k-1} scratch) and the solve is dense mat-vec streaming
-// (bandwidth bound, 2 n_k^2 doubles per level set) interleaved with small sparse products:
-//      forward :  y_k = S_k^-1 (b_k - L_k y_{k-1})
-//      backward:  x_q = y_q,      x_k = y_k - S_k^-1 (U_k x_{k+1})
-// All dense matrices are row-major FP64.
+// the level's block-CSR storage.  The elimination runs from BOTH ends of the chain towards a middle level set m ("burn at
+// both ends"): two independent recurrences, so every step of the solve has two level sets to work on -- twice the bytes per
+// dependent step, which is what makes the solve bandwidth bound instead of latency bound.  Setup (off the solve path)
+// forms the inverses of the Schur complements explicitly,
+//      S_0 = D_0,  S_k = D_k - (L_k S_{k-1}^-1) U_{k-1}  (k < m);      S_q = D_q,  S_k = D_k - (U_k S_{k+1}^-1) L_{k+1}  (k > m);
+//      S_m = D_m - (L_m S_{m-1}^-1) U_{m-1} - (U_m S_{m+1}^-1) L_{m+1},
+// (only S_k^-1 is kept: sum_k n_k^2 doubles plus one n_k x n_{k+-1} scratch) and the solve is dense mat-vec streaming
+// (2 n_k^2 doubles per level set) interleaved with small sparse products:
+//      elimination:       y_k = S_k^-1 (b_k - L_k y_{k-1})  (k < m),    y_k = S_k^-1 (b_k - U_k y_{k+1})  (k > m),
+//                         x_m = S_m^-1 (b_m - L_m y_{m-1} - U_m y_{m+1});
+//      back-substitution: x_k = y_k - S_k^-1 (U_k x_{k+1})  (k < m),    x_k = y_k - S_k^-1 (L_k x_{k-1})  (k > m).
+// Per NEW block row the blocks an elimination step multiplies ("elim" list) and those of the back-substitution ("back"
+// list) are listed at setup.  All dense matrices are row-major FP64.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -102,23 +108,24 @@ __global__ void __launch_bounds__(128) direct_offdiag_kernel(const int64_t *__re
     if (lane == 0) out[row] = (y0 != nullptr ? y0[row] : 0.0) + sign * acc;
 }
 
-// Setup: M (n_k x n_{k-1}) = L_k S_{k-1}^-1 with L_k read from the block-CSR storage.  grid (ceil(n_{k-1} / 128), block
-// rows of level set k); thread = one column of M, 4 scalar rows at a time.
+// Setup: M (n_k x n_kp) = (blocks of level set k with columns in the neighbouring level set kp) S_kp^-1, i.e. L_k S_{k-1}^-1 or
+// U_k S_{k+1}^-1, read from the block-CSR storage.  grid (ceil(n_kp / 128), block rows of level set k); thread = one column
+// of M, 4 scalar rows at a time.
 __global__ void __launch_bounds__(128) direct_lsinv_kernel(const int64_t *__restrict__ row_ptr,
                                                            const int32_t *__restrict__ col_idx,
                                                            const double *__restrict__ vals, const int b, const DirectTables t,
-                                                           const int k, const double *__restrict__ Sprev, const int nprev,
-                                                           double *__restrict__ M) {
+                                                           const int k, const int kp, const double *__restrict__ Sprev,
+                                                           const int nprev, double *__restrict__ M) {
     const int64_t I = t.perm[t.off[k] + blockIdx.y];
     const int c = blockIdx.x * 128 + threadIdx.x;
     if (c >= nprev) return;
     const int64_t p0 = row_ptr[I], p1 = row_ptr[I + 1];
-    const int first_prev = t.off[k - 1];
+    const int first_prev = t.off[kp];
     for (int r0 = 0; r0 < b; r0 += 4) {
         double acc[4] = {0.0, 0.0, 0.0, 0.0};
         for (int64_t p = p0; p < p1; ++p) {
             const int pj = t.inv[col_idx[p]];
-            if (t.lev[pj] != k - 1) continue;
+            if (t.lev[pj] != kp) continue;
             const double *a = vals + (size_t)p * b * b;
             const double *s = Sprev + (size_t)(pj - first_prev) * b * nprev + c;
             for (int q = 0; q < b; ++q) {
@@ -134,16 +141,17 @@ __global__ void __launch_bounds__(128) direct_lsinv_kernel(const int64_t *__rest
     }
 }
 
-// Setup: S_k -= M U_{k-1}.  The blocks of U_{k-1} in block column C of level set k are listed (positions in the block-CSR
-// arrays) in ucsc_pos[ucsc_ptr[new position of C] ...].  grid (block columns of level set k, ceil(n_k / 32)).
+// Setup: S_k -= M X with X = the blocks (row in level set kp, column in level set k), i.e. U_{k-1} or L_{k+1}.  The blocks of X in
+// block column C of level set k are listed (positions in the block-CSR arrays) in csc_pos[csc_ptr[new position of C] ...].
+// grid (block columns of level set k, ceil(n_k / 32)).
 __global__ void __launch_bounds__(128) direct_schur_kernel(const int64_t *__restrict__ ucsc_ptr,
                                                            const int64_t *__restrict__ ucsc_pos,
                                                            const int64_t *__restrict__ row_of_block,
                                                            const double *__restrict__ vals, const int b, const DirectTables t,
-                                                           const int k, const double *__restrict__ M, const int nprev,
-                                                           double *__restrict__ S, const int nk) {
+                                                           const int k, const int kp, const double *__restrict__ M,
+                                                           const int nprev, double *__restrict__ S, const int nk) {
     const int cnew = t.off[k] + blockIdx.x;
-    const int first_prev = t.off[k - 1];
+    const int first_prev = t.off[kp];
     const int64_t u0 = ucsc_ptr[cnew], u1 = ucsc_ptr[cnew + 1];
     for (int idx = threadIdx.x; idx < 32 * b; idx += blockDim.x) {
         const int m = blockIdx.y * 32 + idx / b, cc = idx % b;
@@ -380,57 +388,74 @@ __global__ void permute_blocks_kernel(const double *src, double *dst, const int3
 // ================================================================================================ persistent direct solve
 // ONE cooperative launch per coarsest-level direct solve instead of a chain of ~4 launches per level set.
 //
-//   * grid = one CTA per SM, co-resident (cooperative launch); CTA c owns the contiguous rows [n_k c/G, n_k (c+1)/G) of
-//     every level set k: of the dense inverse S_k^-1 (a contiguous span of the row-major matrix) and of the off-diagonal
-//     block rows L_k / U_k, which the numeric phase packs row by row into a padded (ELL) array in the level-set ordering;
-//   * hence the whole matrix stream of a solve (forward sweep k = 0..q, backward sweep k = q-1..0) is STATIC and contiguous
-//     per CTA and step: one producer warp walks it from start to end with 1-D bulk async copies (TMA engine, SASS UBLKCP)
-//     into a shared-memory ring of DS_SEG-double stages, gated only by the ring's "empty" barriers, and asks for the
-//     stream of the NEXT step to be prefetched into L2 (cp.async.bulk.prefetch.L2) -- a step has four dependent global
-//     round trips (y written -> gathered, t written -> read) of 1-2 us each under load, during which HBM keeps streaming;
-//   * 7 consumer warps per CTA.  Step of level set k:  (A) t = z_k - L_k y_{k-1} (forward) or t = U_k x_{k+1} (backward)
-//     for the CTA's rows, block rows out of the ring, only the gathered y / x values come from global memory;  grid
-//     barrier;  (B) every CTA copies t (n_k doubles) into shared memory and its warps multiply the CTA's rows of S_k^-1
-//     out of the ring (one row per warp at a time, 128-bit shared-memory reads, fixed summation order), writing y_k / x_k;
-//     grid barrier.  The permutation of the right-hand side and of the solution rides in (A) and (B).
+//   * A STEP holds up to two independent jobs (one level set of the lower chain, one of the upper chain; see the top of
+//     this file); a job is (A) the sparse off-diagonal product t = z_k - X y (elimination) or t = X x (back-substitution)
+//     and (B) the dense product with S_k^-1.  The rows of a step's jobs are concatenated and split evenly over the CTAs.
+//   * grid = one CTA per SM, co-resident (cooperative launch); CTA c owns a contiguous row range of every step: of the
+//     dense inverses (contiguous spans of the row-major matrices) and of the off-diagonal block rows, which the numeric
+//     phase packs row by row into a padded (ELL) array in the level-set ordering;
+//   * hence the whole matrix stream of a solve is STATIC and contiguous per CTA and step: one producer warp walks it from
+//     start to end with 1-D bulk async copies (TMA engine, SASS UBLKCP) into a shared-memory ring of DS_SEG-double stages,
+//     gated only by the ring's "empty" barriers: it runs ahead across the steps while the consumers exchange vectors;
+//   * NO grid barrier: the vectors the CTAs exchange (y of the elimination, x of the back-substitution, t of every step)
+//     are written exactly once per solve into buffers that the host fills with a SENTINEL bit pattern (all ones, a NaN
+//     no arithmetic produces) before the launch; a reader polls the values it needs until none is the sentinel (8-byte
+//     accesses at the L2 coherence point).  A dependent step therefore costs two global round trips (y -> gathered by (A),
+//     t -> read by (B)) instead of two barriers plus two round trips, and a CTA waits only for the values it really needs;
+//   * 7 consumer warps per CTA.  (A): DS_TPR threads per scalar row, packed block rows out of the ring, only the gathered
+//     y / x values come from global memory (the column lists were fetched during the preceding step);  (B): every CTA copies
+//     the step's t into shared memory and its warps multiply the CTA's rows of S_k^-1 out of the ring (one row per warp at
+//     a time, 128-bit shared-memory reads, fixed summation order), writing y_k / x_k.  The permutation of the right-hand
+//     side and of the solution rides in (A) and (B).
+// Measured and rejected: grid barriers between (A) and (B) (2.3 ms per C1 solve one-sided, 1.78 ms two-sided: a step is
+// then ~12 us of dependent latency against 10-20 us of streaming); prefetching the stream into L2 ahead of the ring
+// (cp.async.bulk.prefetch.L2, 48 / 160 stages ahead: 6 % / 50 % SLOWER, the L2 -> SM path is not faster than HBM here).
 // Requirements (checked by the host, otherwise the launch chain above is used): b even (16-byte aligned rows for the bulk
-// copies), b <= 64, at most DS_MAXNE listed blocks per block row and side, max n_k doubles + DS_PL ring stages fit the
-// shared memory.
-constexpr int DS_SEG = 1024;            // doubles per ring stage (8 KB)
+// copies), 8 <= b <= 64, at most DS_MAXNE listed blocks per block row and list, the t vectors of a step + DS_PL ring stages +
+// the step table fit the shared memory, the packed stages of one step of one CTA fit the ring together.
+#ifndef MG_DS_SEG
+#define MG_DS_SEG 1024
+#endif
+constexpr int DS_SEG = MG_DS_SEG;       // doubles per ring stage (8 KB)
 constexpr int DS_WARPS = 7;             // consumer warps (+ 1 producer warp = 8: register allocation is per 4 warps)
 constexpr int DS_THREADS = (DS_WARPS + 1) * 32;
 constexpr int DS_PL = 16;               // producer lanes issuing copies in parallel
-constexpr int DS_MAXNE = 16;            // listed blocks per block row and side (ELL width); DS_MAXNE * 64 <= DS_SEG
+constexpr int DS_MAXNE = 16;            // listed blocks per block row and list (ELL width); DS_MAXNE * 64 <= DS_SEG
 constexpr int DS_TPR = 8;               // threads per scalar row in the off-diagonal phase
-constexpr int DS_XCH = 32;              // gathered values a thread keeps in flight
-constexpr int DS_LOOKAHEAD = 48;        // stages (8 KB each, per CTA) the L2 prefetch runs ahead of the shared-memory ring
-constexpr int DS_NCOL = 8;              // column indices of the coming step's row a thread prefetches into registers
-struct DirectLevel {
+constexpr int DS_NCOL = 8;              // listed blocks of a row handled out of registers (more: a second, slower pass)
+struct DsJob {
     const double *S;        // S_k^-1, row-major n x n
-    int n;                  // scalars in the level set
+    long long ell_off;      // offset (doubles) of the job's packed off-diagonal rows [n][ne][b]
+    int n;                  // scalars in the level set (0: no job)
     int first;              // first NEW block position of the level set (scalar offset = first * b)
-    long long ell_off[2];   // offset (doubles) of the level set's packed off-diagonal rows, side 0 = L_k, 1 = U_k
-    int ne[2];              // ELL width of the level set per side (0: no blocks)
+    int ne;                 // ELL width (0: no blocks)
+    int phase;              // 0 elimination (t = z - X y, y = S^-1 t), 1 back-substitution (t = X x, x = y - S^-1 t)
+    int final;              // the job's result is final: scatter it to the natural ordering (and, phase 0, copy it to xb)
+    int toff;               // offset of the job's t in tb
+};
+struct DsStepDesc {
+    DsJob j[2];
 };
 struct DirectSolveArgs {
-    const DirectLevel *lv;   // [nlev]
-    int nlev, b;
-    const double *ell;       // packed off-diagonal rows: [scalar row][ne][b]
-    const int32_t *ell_col;  // [side][new block row][DS_MAXNE] new block column or -1
+    const DsStepDesc *steps;  // [nsteps]
+    int nsteps, b;
+    const double *ell;       // packed off-diagonal rows
+    const int32_t *ell_col;  // [phase][new block row][DS_MAXNE] new block column or -1
     const int32_t *perm;     // block row at NEW position p
     const double *rhs;       // [n] natural ordering
     double *e;               // [n] natural ordering (solution)
-    double *yb, *tb;         // [n] permuted work vectors, [max n_k]
-    unsigned *bar;           // grid barrier counter, zero at launch
+    double *yb, *xb, *tb;    // [n] elimination results, [n] back-substitution results (permuted ordering), [sum of the steps' t];
+                             // all SENTINEL-filled at launch, every entry written once
     int64_t n_brows;
     int stages, tcap;        // ring stages, capacity of the shared-memory copy of t (doubles)
 };
-inline size_t direct_smem_bytes(int stages, int tcap) {
-    return sizeof(double) * ((size_t)stages * DS_SEG + (size_t)tcap) + sizeof(uint64_t) * 2 * (size_t)stages + sizeof(int) * (size_t)stages + 64;
+inline size_t direct_smem_bytes(int stages, int tcap, int nsteps) {
+    return sizeof(double) * ((size_t)stages * DS_SEG + (size_t)tcap) + sizeof(DsStepDesc) * (size_t)nsteps +
+           sizeof(uint64_t) * 2 * (size_t)stages + sizeof(int) * (size_t)stages + 64;
 }
 
-// Numeric phase: pack the listed off-diagonal blocks of every block row (side 0 / 1) into the ELL array of its level set.
-// grid (n_brows, 2); lev_ne / lev_off: [nlev][2].
+// Numeric phase: pack the listed off-diagonal blocks of every block row (list 0 = elimination / 1 = back-substitution) into
+// the ELL array of its level set.  grid (n_brows, 2); lev_ne / lev_off: [nlev][2].
 __global__ void __launch_bounds__(128) direct_pack_ell_kernel(const int64_t *__restrict__ od_ptr0, const int64_t *__restrict__ od_pos0,
                                                               const int32_t *__restrict__ od_col0, const int64_t *__restrict__ od_ptr1,
                                                               const int64_t *__restrict__ od_pos1, const int32_t *__restrict__ od_col1,
@@ -485,73 +510,96 @@ __device__ __forceinline__ void ds_bulk_g2s(void *dst, const void *src, uint32_t
         "l"(src), "r"(bytes), "r"(ds_smem_u32(bar)), "l"(policy)
         : "memory");
 }
-__device__ __forceinline__ void ds_prefetch_l2(const void *src, uint32_t bytes) {
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ unsigned ds_ld_acquire(const unsigned *p) {
-    unsigned v;
-    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+// Sentinel-polled exchange: 8-byte accesses at the L2 coherence point (never L1).
+__device__ __forceinline__ double ds_ld(const double *p) {
+    double v;
+    asm volatile("ld.relaxed.gpu.global.f64 %0, [%1];" : "=d"(v) : "l"(p) : "memory");
     return v;
 }
-// Barrier over the consumer threads of all CTAs of the (co-resident) grid; the producer warps do not take part.
-__device__ __forceinline__ void ds_grid_barrier(unsigned *ctr, unsigned &target, const unsigned nctas) {
-    asm volatile("bar.sync 1, %0;" ::"n"(DS_WARPS * 32) : "memory");
-    if (threadIdx.x == 0) {
-        target += nctas;
-        __threadfence();   // cumulative: orders the writes of the whole CTA (made visible to this thread by bar.sync) before the arrival
-        atomicAdd(ctr, 1u);
-        while (ds_ld_acquire(ctr) < target) {
-        }
-        __threadfence();
-    }
-    asm volatile("bar.sync 1, %0;" ::"n"(DS_WARPS * 32) : "memory");
+__device__ __forceinline__ void ds_st(double *p, const double v) {
+    asm volatile("st.relaxed.gpu.global.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory");
 }
+__device__ __forceinline__ bool ds_missing(const double v) { return __double_as_longlong(v) == -1ll; }
 
-// The stream of one step for one CTA: first the packed off-diagonal rows [ra, rb) of (level k, side), `rps` rows per stage,
-// then the rows [ra, rb) of S_k^-1 in segments of DS_SEG doubles.
-struct DsStep {
+// One CTA's share of one step: per job the rows [ra, rb) of the level set.  Stream order: the packed off-diagonal rows of
+// job 0 (`rps` rows per stage), those of job 1, then the rows of S^-1 of job 0 in segments of DS_SEG doubles, then job 1's.
+struct DsPiece {
     const double *S, *ell;
-    int n, ra, rb, nseg, rowlen, rps, nA, nB;   // rowlen = ne * b doubles per packed row; nA / nB stages
+    int n, first, ra, rb, nseg, rowlen, rps, nA, nB, toff, phase, final;
 };
-__device__ __forceinline__ DsStep ds_step(const DirectSolveArgs &a, const int s, const int c, const int G) {
-    const int nsteps = 2 * a.nlev - 1;
-    const bool fwd = s < a.nlev;
-    const int k = fwd ? s : nsteps - 1 - s;
-    const DirectLevel L = a.lv[k];
-    DsStep d;
-    d.S = L.S;
-    d.n = L.n;
-    d.ra = (int)((long long)L.n * c / G);
-    d.rb = (int)((long long)L.n * (c + 1) / G);
-    d.nseg = (L.n + DS_SEG - 1) / DS_SEG;
-    const int ne = fwd ? L.ne[0] : L.ne[1];
-    d.rowlen = ne * a.b;
-    d.rps = d.rowlen > 0 ? DS_SEG / d.rowlen : 1;
-    d.ell = a.ell + (fwd ? L.ell_off[0] : L.ell_off[1]);
-    d.nA = d.rowlen > 0 ? (d.rb - d.ra + d.rps - 1) / d.rps : 0;
-    d.nB = (d.rb - d.ra) * d.nseg;
-    return d;
+struct DsWork {
+    DsPiece p[2];
+    int nA, total, nt, t0;   // packed stages, all stages, scalars of t in the step, offset of the step's t in tb
+};
+__device__ __forceinline__ DsWork ds_work(const DirectSolveArgs &a, const DsStepDesc &sd, const int c, const int G) {
+    DsWork w;
+    const int n0 = sd.j[0].n, n1 = sd.j[1].n;
+    const int nt = n0 + n1;
+    const int lo = (int)((long long)nt * c / G), hi = (int)((long long)nt * (c + 1) / G);
+    w.nt = nt;
+    w.t0 = sd.j[0].toff;
+    w.nA = 0;
+    w.total = 0;
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+        const DsJob &J = sd.j[q];
+        DsPiece &P = w.p[q];
+        const int base = q ? n0 : 0;
+        P.S = J.S;
+        P.n = J.n;
+        P.first = J.first;
+        P.ra = min(max(lo - base, 0), J.n);
+        P.rb = min(max(hi - base, 0), J.n);
+        P.nseg = (J.n + DS_SEG - 1) / DS_SEG;
+        P.rowlen = J.ne * a.b;
+        P.rps = P.rowlen > 0 ? DS_SEG / P.rowlen : 1;
+        P.ell = a.ell + J.ell_off;
+        P.nA = P.rowlen > 0 ? (P.rb - P.ra + P.rps - 1) / P.rps : 0;
+        P.nB = (P.rb - P.ra) * P.nseg;
+        P.toff = J.toff;
+        P.phase = J.phase;
+        P.final = J.final;
+        w.nA += P.nA;
+        w.total += P.nA + P.nB;
+    }
+    return w;
 }
 // source address and length (doubles) of stage i of a step's stream
-__device__ __forceinline__ const double *ds_stage_src(const DsStep &d, const int i, int &len) {
-    if (i < d.nA) {
-        const int r0 = d.ra + i * d.rps;
-        len = min(d.rps, d.rb - r0) * d.rowlen;
-        return d.ell + (size_t)r0 * d.rowlen;
+__device__ __forceinline__ const double *ds_stage_src(const DsWork &w, int i, int &len) {
+    if (i < w.nA) {
+        DsPiece P = w.p[0];   // (copies selected field by field: an indexed reference would put the struct in local memory)
+        if (i >= w.p[0].nA) {
+            i -= w.p[0].nA;
+            P = w.p[1];
+        }
+        const int r0 = P.ra + i * P.rps;
+        len = min(P.rps, P.rb - r0) * P.rowlen;
+        return P.ell + (size_t)r0 * P.rowlen;
     }
-    const int j = i - d.nA;
-    const int row = d.ra + j / d.nseg, sg = j - (j / d.nseg) * d.nseg;
-    len = min(DS_SEG, d.n - sg * DS_SEG);
-    return d.S + (size_t)row * d.n + (size_t)sg * DS_SEG;
+    i -= w.nA;
+    DsPiece P = w.p[0];
+    if (i >= w.p[0].nB) {
+        i -= w.p[0].nB;
+        P = w.p[1];
+    }
+    const int row = P.ra + i / P.nseg, sg = i - (i / P.nseg) * P.nseg;
+    len = min(DS_SEG, P.n - sg * DS_SEG);
+    return P.S + (size_t)row * P.n + (size_t)sg * DS_SEG;
 }
-
 // column list (first DS_NCOL entries) and permutation entry of NEW block row `pn`: static data
-__device__ __forceinline__ void ds_load_cols(const DirectSolveArgs &a, const int side, const int pn, const bool have, int (&ncol)[DS_NCOL],
+__device__ __forceinline__ void ds_load_cols(const DirectSolveArgs &a, const int phase, const int pn, const bool have, int (&ncol)[DS_NCOL],
                                              int &nperm) {
-    const int32_t *cl = a.ell_col + ((size_t)side * a.n_brows + pn) * DS_MAXNE;
+    const int32_t *cl = a.ell_col + ((size_t)phase * a.n_brows + pn) * DS_MAXNE;
 #pragma unroll
     for (int w = 0; w < DS_NCOL; ++w) ncol[w] = have ? __ldg(cl + w) : -1;
     nperm = have ? __ldg(a.perm + pn) : 0;
+}
+// row q (0-based in the CTA's share of the step) -> piece index and row of the level set; false if q is beyond the share
+__device__ __forceinline__ bool ds_row_of(const DsWork &w, const int q, int &pi, int &row) {
+    const int r0 = w.p[0].rb - w.p[0].ra;
+    pi = q < r0 ? 0 : 1;
+    row = pi == 0 ? w.p[0].ra + q : w.p[1].ra + (q - r0);
+    return q < r0 + (w.p[1].rb - w.p[1].ra);
 }
 
 #ifdef MG_DS_STAMP   // development probe (compiled out in the library): per-phase global-timer stamps of CTA 0
@@ -570,11 +618,13 @@ __global__ void __launch_bounds__(DS_THREADS, 1) direct_solve_persistent_kernel(
     extern __shared__ __align__(128) unsigned char ds_smem[];
     double *ring = reinterpret_cast<double *>(ds_smem);
     double *tsm = ring + (size_t)a.stages * DS_SEG;
-    uint64_t *full = reinterpret_cast<uint64_t *>(tsm + a.tcap);
+    DsStepDesc *steps = reinterpret_cast<DsStepDesc *>(tsm + a.tcap);
+    uint64_t *full = reinterpret_cast<uint64_t *>(steps + a.nsteps);
     uint64_t *empty = full + a.stages;
     volatile int *round_of = reinterpret_cast<volatile int *>(empty + a.stages);   // rounds for which a stage has been issued
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int G = gridDim.x, c = blockIdx.x, b = a.b, ST = a.stages;
+    const int nsteps = a.nsteps;
     if (tid == 0) {
         for (int s = 0; s < ST; ++s) {
             round_of[s] = 0;
@@ -583,41 +633,24 @@ __global__ void __launch_bounds__(DS_THREADS, 1) direct_solve_persistent_kernel(
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    {   // the step table (static) into shared memory: no global round trip at the start of a step
+        const int words = (int)(sizeof(DsStepDesc) / sizeof(int)) * nsteps;
+        const int *src = reinterpret_cast<const int *>(a.steps);
+        int *dst = reinterpret_cast<int *>(steps);
+        for (int i = tid; i < words; i += DS_THREADS) dst[i] = __ldg(src + i);
+    }
     __syncthreads();
-    const int nsteps = 2 * a.nlev - 1;
 
     if (warp == DS_WARPS) {
         // ---------------------------------------------------------------- producer: the CTA's static matrix stream
         uint64_t pol;
         asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
         long long cnt = 0;
-        // L2 prefetch cursor: runs DS_LOOKAHEAD stages ahead of the issue cursor, across step boundaries
-        long long pabs = 0;            // absolute index of the next stage to prefetch
-        int pstep = 0, pidx = 0;
-        DsStep dp = ds_step(a, 0, c, G);
         for (int s = 0; s < nsteps; ++s) {
-            const DsStep d = ds_step(a, s, c, G);
-            const int total = d.nA + d.nB;
-            for (int base = 0; base < total; base += DS_PL) {
-                const long long want = cnt + base + DS_PL + DS_LOOKAHEAD;
-                while (pabs < want && pstep < nsteps) {
-                    const int ptotal = dp.nA + dp.nB;
-                    const int take = (int)min((long long)min(32, ptotal - pidx), want - pabs);
-                    if (take <= 0) {
-                        if (++pstep < nsteps) dp = ds_step(a, pstep, c, G);
-                        pidx = 0;
-                        continue;
-                    }
-                    if (lane < take && pabs + lane >= cnt + base + DS_PL) {   // (stages about to be issued are not worth a prefetch)
-                        int len;
-                        const double *src = ds_stage_src(dp, pidx + lane, len);
-                        ds_prefetch_l2(src, (uint32_t)(len * sizeof(double)));
-                    }
-                    pidx += take;
-                    pabs += take;
-                }
+            const DsWork d = ds_work(a, steps[s], c, G);
+            for (int base = 0; base < d.total; base += DS_PL) {
                 const int i = base + lane;
-                if (lane < DS_PL && i < total) {
+                if (lane < DS_PL && i < d.total) {
                     const long long cc = cnt + i;
                     const int st = (int)(cc % ST);
                     const int round = (int)(cc / ST);
@@ -631,74 +664,94 @@ __global__ void __launch_bounds__(DS_THREADS, 1) direct_solve_persistent_kernel(
                 }
                 __syncwarp();
             }
-            cnt += total;
+            cnt += d.total;
             DS_STAMP(7);
         }
         return;
     }
 
     // -------------------------------------------------------------------- consumers
-    unsigned bar_target = 0;
     long long cnt = 0;
+    constexpr int RPP = DS_WARPS * 32 / DS_TPR;   // rows per pass of phase (A)
+    constexpr int NV = (64 + DS_TPR - 1) / DS_TPR;   // columns of a block per thread (b <= 64)
+    const int sub = tid % DS_TPR;
     int ncol[DS_NCOL], nperm = 0;   // column list / permutation entry of this thread's row in the coming step (first pass)
     {
-        const DsStep d0 = ds_step(a, 0, c, G);
-        const int q = tid / DS_TPR;
-        ds_load_cols(a, 0, a.lv[0].first + (d0.ra + (q < d0.rb - d0.ra ? q : 0)) / b, q < d0.rb - d0.ra, ncol, nperm);
+        const DsWork d0 = ds_work(a, steps[0], c, G);
+        int pi, row;
+        const bool have = ds_row_of(d0, tid / DS_TPR, pi, row);
+        ds_load_cols(a, pi ? d0.p[1].phase : d0.p[0].phase, (pi ? d0.p[1].first : d0.p[0].first) + (have ? row : 0) / b, have, ncol, nperm);
     }
     for (int s = 0; s < nsteps; ++s) {
-        const bool fwd = s < a.nlev;
-        const int k = fwd ? s : nsteps - 1 - s;
-        const DsStep d = ds_step(a, s, c, G);
-        const int first = a.lv[k].first;
+        const DsWork d = ds_work(a, steps[s], c, G);
         DS_STAMP(0);
-        // ---- (A) t = z_k - L_k y_{k-1}   or   t = U_k x_{k+1}   for the rows [ra, rb): DS_TPR threads per scalar row, packed
-        // block rows out of the ring; the column lists (static) were fetched before the preceding grid barrier, so the
-        // gathered y / x values are the only global round trip here, all of a thread's loads in flight at once
+        // ---- (A) t = z_k - X y   or   t = X x   for the CTA's rows: DS_TPR threads per scalar row; thread `sub` of a row takes
+        // the columns sub, sub + DS_TPR, ... of every listed block, all its gathers in flight at once; a gathered value that
+        // is still the sentinel has not been written yet and is loaded again
         {
-            const int nr = d.rb - d.ra;
-            constexpr int RPP = DS_WARPS * 32 / DS_TPR;   // rows per pass
+            const int nr = (d.p[0].rb - d.p[0].ra) + (d.p[1].rb - d.p[1].ra);
             for (int q0 = 0; q0 < nr; q0 += RPP) {
-                const int q = q0 + tid / DS_TPR, sub = tid % DS_TPR;
-                const bool have = q < nr;
-                const int row = d.ra + (have ? q : 0), pl = row / b, r = row - pl * b;
-                if (q0 != 0) ds_load_cols(a, fwd ? 0 : 1, first + pl, have, ncol, nperm);
-                double acc = 0.0;
-                double zv = 0.0;
-                if (have && fwd) zv = __ldg(a.rhs + (size_t)nperm * b + r);
-                if (have && d.rowlen > 0) {
-                    const long long cc = cnt + q / d.rps;
+                int pi, row;
+                const bool have = ds_row_of(d, q0 + tid / DS_TPR, pi, row);
+                DsPiece P = d.p[0];
+                if (pi) P = d.p[1];
+                if (!have) row = P.ra;
+                const int pl = row / b, r = row - pl * b;
+                if (q0 != 0) ds_load_cols(a, P.phase, P.first + pl, have, ncol, nperm);
+                double acc = 0.0, zv = 0.0;
+                if (have && P.phase == 0) zv = __ldg(a.rhs + (size_t)nperm * b + r);
+                if (have && P.rowlen > 0) {
+                    const double *src = P.phase == 0 ? a.yb : a.xb;
+                    const int ne = P.rowlen / b;
+                    double xv[DS_NCOL][NV];
+#pragma unroll
+                    for (int w = 0; w < DS_NCOL; ++w)
+#pragma unroll
+                        for (int v = 0; v < NV; ++v) {
+                            const int cx = sub + v * DS_TPR;
+                            xv[w][v] = (w < ne && ncol[w] >= 0 && cx < b) ? ds_ld(src + (size_t)ncol[w] * b + cx) : 0.0;
+                        }
+                    bool again;
+                    do {
+                        again = false;
+#pragma unroll
+                        for (int w = 0; w < DS_NCOL; ++w)
+#pragma unroll
+                            for (int v = 0; v < NV; ++v)
+                                if (ds_missing(xv[w][v])) {
+                                    xv[w][v] = ds_ld(src + (size_t)ncol[w] * b + sub + v * DS_TPR);
+                                    again = again || ds_missing(xv[w][v]);
+                                }
+                    } while (again);
+                    const int ql = row - P.ra;                       // row within the piece
+                    const long long cc = cnt + (pi ? d.p[0].nA : 0) + ql / P.rps;
                     const int st = (int)(cc % ST);
                     const int round = (int)(cc / ST);
                     while (round_of[st] <= round) __nanosleep(100);
                     while (!ds_mbar_try(&full[st], (uint32_t)round & 1u)) {
                     }
-                    const double *As = ring + (size_t)st * DS_SEG + (size_t)(q - (q / d.rps) * d.rps) * d.rowlen;
-                    for (int f0 = sub; f0 < d.rowlen; f0 += DS_TPR * DS_XCH) {
-                        double xv[DS_XCH];
+                    const double *As = ring + (size_t)st * DS_SEG + (size_t)(ql - (ql / P.rps) * P.rps) * P.rowlen;
 #pragma unroll
-                        for (int u = 0; u < DS_XCH; ++u) {
-                            const int f = f0 + u * DS_TPR;
-                            xv[u] = 0.0;
-                            if (f < d.rowlen) {
-                                const int ie = f / b, cx = f - ie * b;
-                                int col = -1;
+                    for (int w = 0; w < DS_NCOL; ++w)
 #pragma unroll
-                                for (int w = 0; w < DS_NCOL; ++w) col = (ie == w) ? ncol[w] : col;
-                                if (ie >= DS_NCOL) col = __ldg(a.ell_col + ((size_t)(fwd ? 0 : 1) * a.n_brows + first + pl) * DS_MAXNE + ie);
-                                if (col >= 0) xv[u] = __ldcg(a.yb + (size_t)col * b + cx);
+                        for (int v = 0; v < NV; ++v) {
+                            const int cx = sub + v * DS_TPR;
+                            if (w < ne && cx < b) acc = fma(As[w * b + cx], xv[w][v], acc);
+                        }
+                    for (int w = DS_NCOL; w < ne; ++w) {   // rows with more listed blocks than registers hold: the plain way
+                        const int col = __ldg(a.ell_col + ((size_t)P.phase * a.n_brows + P.first + pl) * DS_MAXNE + w);
+                        if (col >= 0)
+                            for (int cx = sub; cx < b; cx += DS_TPR) {
+                                double x1;
+                                do x1 = ds_ld(src + (size_t)col * b + cx);
+                                while (ds_missing(x1));
+                                acc = fma(As[w * b + cx], x1, acc);
                             }
-                        }
-#pragma unroll
-                        for (int u = 0; u < DS_XCH; ++u) {
-                            const int f = f0 + u * DS_TPR;
-                            if (f < d.rowlen) acc = fma(As[f], xv[u], acc);
-                        }
                     }
                 }
 #pragma unroll
                 for (int o = DS_TPR / 2; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-                if (have && sub == 0) a.tb[row] = fwd ? zv - acc : acc;
+                if (have && sub == 0) ds_st(a.tb + P.toff + row, P.phase == 0 ? zv - acc : acc);
             }
         }
         // all rows of the step's packed stages are consumed once every consumer warp is here: hand the stages back
@@ -706,78 +759,101 @@ __global__ void __launch_bounds__(DS_THREADS, 1) direct_solve_persistent_kernel(
         for (int i = tid; i < d.nA; i += DS_WARPS * 32) ds_mbar_arrive(&empty[(int)((cnt + i) % ST)]);
         cnt += d.nA;
         DS_STAMP(1);
-        ds_grid_barrier(a.bar, bar_target, (unsigned)G);
-        DS_STAMP(2);
-        // ---- (B) rows of S_k^-1 times t
-        for (int i0 = 0; i0 < d.n; i0 += 8 * 2 * DS_WARPS * 32) {   // 8 independent 128-bit loads in flight per thread (n even)
-            double2 tv[8];
+        // ---- (B) rows of S_k^-1 times t: the step's t (written by all CTAs) into shared memory, polled until complete
+        for (int i0 = 0; i0 < d.nt; i0 += 16 * DS_WARPS * 32) {   // 16 independent loads in flight per thread
+            double tv[16];
 #pragma unroll
-            for (int u = 0; u < 8; ++u) {
-                const int i = i0 + 2 * (tid + u * DS_WARPS * 32);
-                tv[u] = i < d.n ? __ldcg(reinterpret_cast<const double2 *>(a.tb + i)) : make_double2(0.0, 0.0);
+            for (int u = 0; u < 16; ++u) {
+                const int i = i0 + tid + u * DS_WARPS * 32;
+                tv[u] = i < d.nt ? ds_ld(a.tb + d.t0 + i) : 0.0;
             }
+            bool again;
+            do {
+                again = false;
 #pragma unroll
-            for (int u = 0; u < 8; ++u) {
-                const int i = i0 + 2 * (tid + u * DS_WARPS * 32);
-                if (i < d.n) *reinterpret_cast<double2 *>(tsm + i) = tv[u];
+                for (int u = 0; u < 16; ++u)
+                    if (ds_missing(tv[u])) {
+                        tv[u] = ds_ld(a.tb + d.t0 + i0 + tid + u * DS_WARPS * 32);
+                        again = again || ds_missing(tv[u]);
+                    }
+            } while (again);
+#pragma unroll
+            for (int u = 0; u < 16; ++u) {
+                const int i = i0 + tid + u * DS_WARPS * 32;
+                if (i < d.nt) tsm[i] = tv[u];
             }
         }
         asm volatile("bar.sync 1, %0;" ::"n"(DS_WARPS * 32) : "memory");
         DS_STAMP(3);
-        for (int i = warp; i < d.rb - d.ra; i += DS_WARPS) {
-            const int row = d.ra + i;
-            double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
-            for (int sg = 0; sg < d.nseg; ++sg) {
-                const long long cc = cnt + (long long)i * d.nseg + sg;
-                const int st = (int)(cc % ST);
-                const int round = (int)(cc / ST);
-                while (round_of[st] <= round) __nanosleep(100);
-                while (!ds_mbar_try(&full[st], (uint32_t)round & 1u)) {
+        {
+            const int nr0 = d.p[0].rb - d.p[0].ra, nr = nr0 + (d.p[1].rb - d.p[1].ra);
+            for (int i = warp; i < nr; i += DS_WARPS) {
+                const int pi = i < nr0 ? 0 : 1;
+                DsPiece P = d.p[0];
+                if (pi) P = d.p[1];
+                const int il = pi ? i - nr0 : i;
+                const int row = P.ra + il;
+                const long long c0 = cnt + (pi ? d.p[0].nB : 0) + (long long)il * P.nseg;
+                double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+                for (int sg = 0; sg < P.nseg; ++sg) {
+                    const long long cc = c0 + sg;
+                    const int st = (int)(cc % ST);
+                    const int round = (int)(cc / ST);
+                    while (round_of[st] <= round) __nanosleep(100);
+                    while (!ds_mbar_try(&full[st], (uint32_t)round & 1u)) {
+                    }
+                    const int len2 = min(DS_SEG, P.n - sg * DS_SEG) >> 1;
+                    const double2 *A2 = reinterpret_cast<const double2 *>(ring + (size_t)st * DS_SEG);
+                    const double2 *t2 = reinterpret_cast<const double2 *>(tsm + (P.toff - d.t0) + (size_t)sg * DS_SEG);
+                    int e = lane;
+                    for (; e + 32 < len2; e += 64) {
+                        const double2 v0 = A2[e], v1 = A2[e + 32];
+                        const double2 y0 = t2[e], y1 = t2[e + 32];
+                        s0 = fma(v0.x, y0.x, s0);
+                        s1 = fma(v0.y, y0.y, s1);
+                        s2 = fma(v1.x, y1.x, s2);
+                        s3 = fma(v1.y, y1.y, s3);
+                    }
+                    if (e < len2) {
+                        const double2 v0 = A2[e], y0 = t2[e];
+                        s0 = fma(v0.x, y0.x, s0);
+                        s1 = fma(v0.y, y0.y, s1);
+                    }
+                    __syncwarp();
+                    if (lane == 0) ds_mbar_arrive(&empty[st]);
                 }
-                const int len2 = min(DS_SEG, d.n - sg * DS_SEG) >> 1;
-                const double2 *A2 = reinterpret_cast<const double2 *>(ring + (size_t)st * DS_SEG);
-                const double2 *t2 = reinterpret_cast<const double2 *>(tsm + (size_t)sg * DS_SEG);
-                int e = lane;
-                for (; e + 32 < len2; e += 64) {
-                    const double2 v0 = A2[e], v1 = A2[e + 32];
-                    const double2 y0 = t2[e], y1 = t2[e + 32];
-                    s0 = fma(v0.x, y0.x, s0);
-                    s1 = fma(v0.y, y0.y, s1);
-                    s2 = fma(v1.x, y1.x, s2);
-                    s3 = fma(v1.y, y1.y, s3);
-                }
-                if (e < len2) {
-                    const double2 v0 = A2[e], y0 = t2[e];
-                    s0 = fma(v0.x, y0.x, s0);
-                    s1 = fma(v0.y, y0.y, s1);
-                }
-                __syncwarp();
-                if (lane == 0) ds_mbar_arrive(&empty[st]);
-            }
-            double sum = (s0 + s1) + (s2 + s3);
+                double sum = (s0 + s1) + (s2 + s3);
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
-            if (lane == 0) {
-                const size_t gi = (size_t)first * b + row;
-                const double yv = fwd ? sum : __ldcg(a.yb + gi) - sum;
-                a.yb[gi] = yv;
-                if (!fwd || k == a.nlev - 1) {   // final value of this row: scatter to the natural ordering
-                    const int pl = row / b;
-                    a.e[(size_t)__ldg(a.perm + first + pl) * b + (row - pl * b)] = yv;
+                for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+                if (lane == 0) {
+                    const size_t gi = (size_t)P.first * b + row;
+                    if (P.phase == 0) {
+                        ds_st(a.yb + gi, sum);
+                        if (P.final) ds_st(a.xb + gi, sum);   // the middle level set: its result is also the first x
+                    } else {
+                        double yk;                            // y_k of the elimination phase (written many steps ago, possibly
+                        do yk = ds_ld(a.yb + gi);             // by another CTA: the steps pair the level sets differently)
+                        while (ds_missing(yk));
+                        sum = yk - sum;
+                        ds_st(a.xb + gi, sum);
+                    }
+                    if (P.final) {   // final value of this row: scatter to the natural ordering
+                        const int pl = row / b;
+                        a.e[(size_t)__ldg(a.perm + P.first + pl) * b + (row - pl * b)] = sum;
+                    }
                 }
             }
         }
-        cnt += d.nB;
+        cnt += d.p[0].nB + d.p[1].nB;
         DS_STAMP(4);
-        if (s + 1 < nsteps) {   // static data of the coming step's first pass, fetched behind the grid barrier
-            const DsStep dn = ds_step(a, s + 1, c, G);
-            const bool fn = s + 1 < a.nlev;
-            const int kn = fn ? s + 1 : nsteps - 2 - s;
-            const int q = tid / DS_TPR;
-            ds_load_cols(a, fn ? 0 : 1, a.lv[kn].first + (dn.ra + (q < dn.rb - dn.ra ? q : 0)) / b, q < dn.rb - dn.ra, ncol, nperm);
+        if (s + 1 < nsteps) {   // static data of the coming step's first pass
+            const DsWork dn = ds_work(a, steps[s + 1], c, G);
+            int pi, row;
+            const bool have = ds_row_of(dn, tid / DS_TPR, pi, row);
+            ds_load_cols(a, pi ? dn.p[1].phase : dn.p[0].phase, (pi ? dn.p[1].first : dn.p[0].first) + (have ? row : 0) / b, have, ncol, nperm);
         }
-        DS_STAMP(5);
-        ds_grid_barrier(a.bar, bar_target, (unsigned)G);
+        // tsm is rewritten in the next step: every warp must be done reading it
+        asm volatile("bar.sync 1, %0;" ::"n"(DS_WARPS * 32) : "memory");
         DS_STAMP(6);
     }
 }

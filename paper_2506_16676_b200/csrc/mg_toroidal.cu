@@ -82,9 +82,13 @@ struct DirectCoarse {
     double *Mtmp = nullptr;     // scratch of the numeric phase: L_k S_{k-1}^-1
     int32_t *perm = nullptr, *inv = nullptr, *lev = nullptr, *off = nullptr;   // device
     double **dS = nullptr;      // device pointer table
-    int64_t *ucsc_ptr = nullptr, *ucsc_pos = nullptr;   // blocks of U_{k-1} by block column (new numbering)
-    int64_t *od_ptr[2] = {nullptr, nullptr}, *od_pos[2] = {nullptr, nullptr};   // blocks of L_k (0) / U_k (1) by block row
-    int32_t *od_col[2] = {nullptr, nullptr};                                    // (new numbering) and their new columns
+    int mid = 0;                // middle level set: elimination runs 0 -> mid and nlev-1 -> mid
+    int64_t *csc_ptr[2] = {nullptr, nullptr}, *csc_pos[2] = {nullptr, nullptr};   // by block column (new numbering): 0 = blocks of U_{k-1}
+                                // (row one level set down), 1 = blocks of L_{k+1} (row one level set up): the Schur updates
+    int64_t *od_ptr[2] = {nullptr, nullptr}, *od_pos[2] = {nullptr, nullptr};   // by block row (new numbering): 0 = the blocks an
+    int32_t *od_col[2] = {nullptr, nullptr};   // elimination step multiplies, 1 = those of the back-substitution; new columns
+    struct Job { int level, phase, final; };
+    std::vector<std::vector<Job>> steps;       // the solve: steps of up to two independent jobs
     int64_t *rob = nullptr;     // block row of every stored block
     double *zb = nullptr, *yb = nullptr, *tb = nullptr;
     double *pinv = nullptr, *cpanel = nullptr, *rpanel = nullptr;   // blocked Gauss-Jordan: pivot-block inverse, saved panels
@@ -93,8 +97,9 @@ struct DirectCoarse {
     int64_t bytes = 0;
     // persistent cooperative solve kernel (direct_solve_persistent_kernel); the launch chain is the fallback
     bool persist = false;
-    DirectLevel *lvdev = nullptr;
-    unsigned *bar = nullptr;
+    DsStepDesc *stepdev = nullptr;
+    double *xchg = nullptr;       // yb | xb | tb of the persistent kernel, one allocation (sentinel-filled before every launch)
+    int64_t xchg_doubles = 0, tb_doubles = 0;
     int ds_grid = 0, ds_stages = 0, ds_tcap = 0;
     size_t ds_smem = 0;
     std::vector<int32_t> first;   // first new block position of every level set
@@ -791,38 +796,50 @@ int direct_symbolic(mg_handle *h) {
             lev_new[pnew] = lev_of_old[i];
         }
     }
-    // every block must couple equal or adjacent level sets (true for a structurally symmetric pattern); the blocks of
-    // U_{k-1} (row in level set k-1, column in level set k) are listed by block column for the Schur update
-    std::vector<int64_t> ucsc_ptr((size_t)n + 1, 0), ucsc_pos;
+    // every block must couple equal or adjacent level sets (true for a structurally symmetric pattern)
     for (int64_t i = 0; i < n; ++i)
         for (int64_t p = L.h_row_ptr[i]; p < L.h_row_ptr[i + 1]; ++p) {
-            const int64_t j = L.h_col_idx[p];
-            const int d = lev_of_old[j] - lev_of_old[i];
+            const int d = lev_of_old[L.h_col_idx[p]] - lev_of_old[i];
             if (d > 1 || d < -1) return MG_EINVAL;
-            if (d == 1) ucsc_ptr[inv[j] + 1]++;
         }
-    for (int64_t i = 0; i < n; ++i) ucsc_ptr[i + 1] += ucsc_ptr[i];
-    ucsc_pos.resize((size_t)std::max<int64_t>(ucsc_ptr[n], 1));
-    {
-        std::vector<int64_t> cur(ucsc_ptr.begin(), ucsc_ptr.end() - 1);
+    // Two-sided elimination: level sets 0 .. mid-1 are eliminated upwards, nlev-1 .. mid+1 downwards, mid last.
+    dc.mid = dc.nlev / 2;
+    const int mid = dc.mid;
+    // blocks by block column for the Schur updates: list 0 = (row one level set DOWN, i.e. U_{k-1}), 1 = (row one level set UP, L_{k+1})
+    std::vector<int64_t> csc_ptr[2], csc_pos[2];
+    for (int dir = 0; dir < 2; ++dir) {
+        const int want = dir == 0 ? 1 : -1;   // lev(col) - lev(row)
+        csc_ptr[dir].assign((size_t)n + 1, 0);
         for (int64_t i = 0; i < n; ++i)
             for (int64_t p = L.h_row_ptr[i]; p < L.h_row_ptr[i + 1]; ++p) {
                 const int64_t j = L.h_col_idx[p];
-                if (lev_of_old[j] - lev_of_old[i] == 1) ucsc_pos[cur[inv[j]]++] = p;
+                if (lev_of_old[j] - lev_of_old[i] == want) csc_ptr[dir][inv[j] + 1]++;
+            }
+        for (int64_t i = 0; i < n; ++i) csc_ptr[dir][i + 1] += csc_ptr[dir][i];
+        csc_pos[dir].resize((size_t)std::max<int64_t>(csc_ptr[dir][n], 1));
+        std::vector<int64_t> cur(csc_ptr[dir].begin(), csc_ptr[dir].end() - 1);
+        for (int64_t i = 0; i < n; ++i)
+            for (int64_t p = L.h_row_ptr[i]; p < L.h_row_ptr[i + 1]; ++p) {
+                const int64_t j = L.h_col_idx[p];
+                if (lev_of_old[j] - lev_of_old[i] == want) csc_pos[dir][cur[inv[j]]++] = p;
             }
     }
-    // row-wise lists of the off-diagonal blocks for the solve: side 0 = L (column one level set down), 1 = U (one up)
+    // row-wise lists of the off-diagonal blocks for the solve: list 0 = elimination (columns in the level set eliminated just
+    // before: k-1 below mid, k+1 above, both at mid), list 1 = back-substitution (the other neighbour; none at mid)
     std::vector<int64_t> od_ptr[2], od_pos[2];
     std::vector<int32_t> od_col[2];
     dc.offdiag_blocks = 0;
     for (int side = 0; side < 2; ++side) {
-        const int want = side == 0 ? -1 : 1;
         od_ptr[side].assign((size_t)n + 1, 0);
         for (int64_t pn = 0; pn < n; ++pn) {
             const int64_t i = perm[pn];
+            const int k = lev_of_old[i];
             for (int64_t p = L.h_row_ptr[i]; p < L.h_row_ptr[i + 1]; ++p) {
                 const int64_t j = L.h_col_idx[p];
-                if (lev_of_old[j] - lev_of_old[i] != want) continue;
+                const int d = lev_of_old[j] - k;
+                if (d == 0) continue;
+                const bool elim = (k < mid && d == -1) || (k > mid && d == 1) || k == mid;
+                if ((side == 0) != elim) continue;
                 od_pos[side].push_back(p);
                 od_col[side].push_back(inv[j]);
             }
@@ -834,6 +851,24 @@ int direct_symbolic(mg_handle *h) {
             od_col[side].push_back(0);
         }
     }
+    // steps of the solve: elimination from both ends, the middle level set, back-substitution outwards
+    dc.steps.clear();
+    {
+        const int q = dc.nlev - 1;
+        for (int j = 0; j < std::max(mid, q - mid); ++j) {
+            std::vector<DirectCoarse::Job> st;
+            if (j < mid) st.push_back({j, 0, 0});
+            if (q - j > mid) st.push_back({q - j, 0, 0});
+            dc.steps.push_back(st);
+        }
+        dc.steps.push_back({{mid, 0, 1}});
+        for (int j = 1; j <= std::max(mid, q - mid); ++j) {
+            std::vector<DirectCoarse::Job> st;
+            if (mid - j >= 0) st.push_back({mid - j, 1, 1});
+            if (mid + j <= q) st.push_back({mid + j, 1, 1});
+            dc.steps.push_back(st);
+        }
+    }
     dc.nk.resize(dc.nlev);
     dc.voff.assign(dc.nlev + 1, 0);
     dc.maxn = 0;
@@ -843,8 +878,8 @@ int direct_symbolic(mg_handle *h) {
         dc.voff[k + 1] = dc.voff[k] + dc.nk[k];
         dc.maxn = std::max(dc.maxn, dc.nk[k]);
         bytes += (int64_t)sizeof(double) * dc.nk[k] * dc.nk[k];
-        if (k > 0) mtmp = std::max(mtmp, (int64_t)dc.nk[k] * dc.nk[k - 1]);
     }
+    for (int k = 1; k < dc.nlev; ++k) mtmp = std::max(mtmp, (int64_t)dc.nk[k] * dc.nk[k - 1]);
     bytes += (int64_t)sizeof(double) * mtmp;
     size_t free_b = 0, total_b = 0;
     CU(cudaMemGetInfo(&free_b, &total_b));
@@ -858,9 +893,12 @@ int direct_symbolic(mg_handle *h) {
     MG(dalloc_t(h, &dc.lev, (size_t)n));
     MG(dalloc_t(h, &dc.off, (size_t)dc.nlev + 1));
     MG(dalloc_t(h, &dc.dS, (size_t)dc.nlev));
-    MG(dalloc_t(h, &dc.ucsc_ptr, (size_t)n + 1));
-    MG(dalloc_t(h, &dc.ucsc_pos, ucsc_pos.size()));
     for (int side = 0; side < 2; ++side) {
+        MG(dalloc_t(h, &dc.csc_ptr[side], (size_t)n + 1));
+        MG(dalloc_t(h, &dc.csc_pos[side], csc_pos[side].size()));
+        CU(cudaMemcpyAsync(dc.csc_ptr[side], csc_ptr[side].data(), sizeof(int64_t) * (n + 1), cudaMemcpyHostToDevice, h->stream));
+        CU(cudaMemcpyAsync(dc.csc_pos[side], csc_pos[side].data(), sizeof(int64_t) * csc_pos[side].size(), cudaMemcpyHostToDevice,
+                           h->stream));
         MG(dalloc_t(h, &dc.od_ptr[side], (size_t)n + 1));
         MG(dalloc_t(h, &dc.od_pos[side], od_pos[side].size()));
         MG(dalloc_t(h, &dc.od_col[side], od_col[side].size()));
@@ -872,7 +910,7 @@ int direct_symbolic(mg_handle *h) {
     }
     MG(dalloc_t(h, &dc.zb, (size_t)L.nvec + 2));
     MG(dalloc_t(h, &dc.yb, (size_t)L.nvec + 2));
-    MG(dalloc_t(h, &dc.tb, (size_t)dc.maxn + 2));
+    MG(dalloc_t(h, &dc.tb, (size_t)2 * dc.maxn + 2));
     MG(dalloc_t(h, &dc.pinv, (size_t)GJ_W * GJ_W));
     MG(dalloc_t(h, &dc.cpanel, (size_t)dc.maxn * GJ_W + 2));
     MG(dalloc_t(h, &dc.rpanel, (size_t)dc.maxn * GJ_W + 2));
@@ -882,8 +920,6 @@ int direct_symbolic(mg_handle *h) {
     CU(cudaMemcpyAsync(dc.lev, lev_new.data(), sizeof(int32_t) * n, cudaMemcpyHostToDevice, h->stream));
     CU(cudaMemcpyAsync(dc.off, off.data(), sizeof(int32_t) * (dc.nlev + 1), cudaMemcpyHostToDevice, h->stream));
     CU(cudaMemcpyAsync(dc.dS, dc.S.data(), sizeof(double *) * dc.nlev, cudaMemcpyHostToDevice, h->stream));
-    CU(cudaMemcpyAsync(dc.ucsc_ptr, ucsc_ptr.data(), sizeof(int64_t) * (n + 1), cudaMemcpyHostToDevice, h->stream));
-    CU(cudaMemcpyAsync(dc.ucsc_pos, ucsc_pos.data(), sizeof(int64_t) * ucsc_pos.size(), cudaMemcpyHostToDevice, h->stream));
     if (L.row_of_block != nullptr) dc.rob = L.row_of_block;
     else {
         MG(dalloc_t(h, &dc.rob, (size_t)std::max<int64_t>(L.nnzb, 1)));
@@ -910,50 +946,73 @@ int direct_symbolic(mg_handle *h) {
                 lev_off[2 * k + side] = ell_doubles;
                 ell_doubles += (long long)dc.nk[k] * lev_ne[2 * k + side] * b;
             }
-        const int tcap = (dc.maxn + 1) / 2 * 2;
+        const int nsteps = (int)dc.steps.size();
+        int tcap = 2;
+        for (const auto &st : dc.steps) {
+            int nt = 0;
+            for (const auto &j : st) nt += dc.nk[j.level];
+            tcap = std::max(tcap, (nt + 1) / 2 * 2);
+        }
         const size_t budget = 227 * 1024;
         int stages = 0;
-        if (direct_smem_bytes(DS_PL, tcap) <= budget)
-            stages = (int)std::min<size_t>(64, (budget - direct_smem_bytes(0, tcap)) / (sizeof(double) * DS_SEG + 2 * sizeof(uint64_t) + sizeof(int)));
-        bool fits = (b % 2 == 0) && b <= 64 && ne_max <= DS_MAXNE && stages >= DS_PL && h->coop_launch;
-        for (int k = 0; fits && k < dc.nlev; ++k)
-            for (int side = 0; side < 2; ++side) {
-                const int rowlen = lev_ne[2 * k + side] * b;
+        if (direct_smem_bytes(DS_PL, tcap, nsteps) <= budget)
+            stages = (int)std::min<size_t>(64, (budget - direct_smem_bytes(0, tcap, nsteps)) /
+                                                   (sizeof(double) * DS_SEG + 2 * sizeof(uint64_t) + sizeof(int)));
+        bool fits = (b % 2 == 0) && b >= DS_TPR && b <= 64 && ne_max <= DS_MAXNE && stages >= DS_PL && h->coop_launch;
+        for (size_t si = 0; fits && si < dc.steps.size(); ++si) {   // the packed stages of a step are handed back together
+            int nA = 0;
+            for (const auto &j : dc.steps[si]) {
+                const int rowlen = lev_ne[2 * j.level + j.phase] * b;
                 if (rowlen == 0) continue;
-                const int rps = DS_SEG / rowlen, nr = dc.nk[k] / h->sm_count + 2;
-                if (rps < 1 || (nr + rps - 1) / rps > stages - 1) fits = false;
+                const int rps = DS_SEG / rowlen, nr = dc.nk[j.level] / h->sm_count + 2;
+                if (rps < 1) fits = false;
+                else nA += (nr + rps - 1) / rps;
             }
+            if (nA > stages - 1) fits = false;
+        }
         int per_sm = 0;
         if (fits &&
             cudaFuncSetAttribute(direct_solve_persistent_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)direct_smem_bytes(stages, tcap)) == cudaSuccess &&
+                                 (int)direct_smem_bytes(stages, tcap, nsteps)) == cudaSuccess &&
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, direct_solve_persistent_kernel, DS_THREADS,
-                                                          direct_smem_bytes(stages, tcap)) == cudaSuccess && per_sm >= 1) {
+                                                          direct_smem_bytes(stages, tcap, nsteps)) == cudaSuccess && per_sm >= 1) {
             dc.ds_stages = stages;
             dc.ds_tcap = tcap;
-            dc.ds_smem = direct_smem_bytes(stages, tcap);
+            dc.ds_smem = direct_smem_bytes(stages, tcap, nsteps);
             dc.ds_grid = h->sm_count;
             dc.ell_doubles = ell_doubles;
-            MG(dalloc_t(h, &dc.lvdev, (size_t)dc.nlev));
-            MG(dalloc_t(h, &dc.bar, 4));
+            MG(dalloc_t(h, &dc.stepdev, (size_t)nsteps));
             MG(dalloc_t(h, &dc.ell, (size_t)std::max<long long>(ell_doubles, 2)));
             MG(dalloc_t(h, &dc.ell_col, (size_t)2 * n * DS_MAXNE));
             MG(dalloc_t(h, &dc.lev_ne, (size_t)2 * dc.nlev));
             MG(dalloc_t(h, &dc.lev_off, (size_t)2 * dc.nlev));
-            std::vector<DirectLevel> lv((size_t)dc.nlev);
-            for (int k = 0; k < dc.nlev; ++k) {
-                lv[k].S = dc.S[k];
-                lv[k].n = dc.nk[k];
-                lv[k].first = off[k];
-                for (int side = 0; side < 2; ++side) {
-                    lv[k].ell_off[side] = lev_off[2 * k + side];
-                    lv[k].ne[side] = lev_ne[2 * k + side];
+            std::vector<DsStepDesc> sd((size_t)nsteps);
+            std::memset(sd.data(), 0, sizeof(DsStepDesc) * sd.size());
+            int64_t toff = 0;
+            for (int si = 0; si < nsteps; ++si)
+                for (size_t ji = 0; ji < 2; ++ji) {
+                    if (ji >= dc.steps[si].size()) {
+                        sd[si].j[ji].toff = (int)toff;
+                        continue;
+                    }
+                    const auto &j = dc.steps[si][ji];
+                    DsJob &J = sd[si].j[ji];
+                    J.S = dc.S[j.level];
+                    J.ell_off = lev_off[2 * j.level + j.phase];
+                    J.n = dc.nk[j.level];
+                    J.first = off[j.level];
+                    J.ne = lev_ne[2 * j.level + j.phase];
+                    J.phase = j.phase;
+                    J.final = j.final;
+                    J.toff = (int)toff;
+                    toff += J.n;
                 }
-            }
-            CU(cudaMemcpyAsync(dc.lvdev, lv.data(), sizeof(DirectLevel) * dc.nlev, cudaMemcpyHostToDevice, h->stream));
+            dc.tb_doubles = toff;
+            dc.xchg_doubles = 2 * (int64_t)L.nvec + toff;
+            MG(dalloc_t(h, &dc.xchg, (size_t)dc.xchg_doubles + 2));
+            CU(cudaMemcpyAsync(dc.stepdev, sd.data(), sizeof(DsStepDesc) * nsteps, cudaMemcpyHostToDevice, h->stream));
             CU(cudaMemcpyAsync(dc.lev_ne, lev_ne.data(), sizeof(int) * 2 * dc.nlev, cudaMemcpyHostToDevice, h->stream));
             CU(cudaMemcpyAsync(dc.lev_off, lev_off.data(), sizeof(long long) * 2 * dc.nlev, cudaMemcpyHostToDevice, h->stream));
-            CU(cudaMemsetAsync(dc.yb, 0, sizeof(double) * ((size_t)L.nvec + 2), h->stream));
             CU(cudaStreamSynchronize(h->stream));
             dc.persist = true;
         } else {
@@ -991,17 +1050,28 @@ int direct_numeric(mg_handle *h) {
     DirectTables t{dc.perm, dc.inv, dc.lev, dc.off, dc.dS};
     if (L.nnzb > 0) LAUNCH(h, direct_assemble_kernel, (unsigned)L.nnzb, 128, 0, dc.rob, L.col_idx, L.vals, b, t);
     CU(cudaGetLastError());
-    for (int k = 0; k < dc.nlev; ++k) {
-        if (k > 0) {
-            const int nk = dc.nk[k], np = dc.nk[k - 1];
-            LAUNCH(h, direct_lsinv_kernel, dim3((np + 127) / 128, nk / b), 128, 0, L.row_ptr, L.col_idx, L.vals, b, t, k,
-                   dc.S[k - 1], np, dc.Mtmp);
-            LAUNCH(h, direct_schur_kernel, dim3(nk / b, (nk + 31) / 32), 128, 0, dc.ucsc_ptr, dc.ucsc_pos, dc.rob, L.vals, b, t, k,
-                   dc.Mtmp, np, dc.S[k], nk);
-            CU(cudaGetLastError());
-        }
+    // S_k -= (blocks of level set k with columns in kp) S_kp^-1 (blocks with rows in kp and columns in k); S_kp^-1 is final
+    auto schur_update = [&](int k, int kp) -> int {
+        const int nk = dc.nk[k], np = dc.nk[kp];
+        const int dir = kp < k ? 0 : 1;
+        LAUNCH(h, direct_lsinv_kernel, dim3((np + 127) / 128, nk / b), 128, 0, L.row_ptr, L.col_idx, L.vals, b, t, k, kp, dc.S[kp], np,
+               dc.Mtmp);
+        LAUNCH(h, direct_schur_kernel, dim3(nk / b, (nk + 31) / 32), 128, 0, dc.csc_ptr[dir], dc.csc_pos[dir], dc.rob, L.vals, b, t, k, kp,
+               dc.Mtmp, np, dc.S[k], nk);
+        CU(cudaGetLastError());
+        return MG_OK;
+    };
+    for (int k = 0; k < dc.mid; ++k) {            // lower chain, upwards
+        if (k > 0) MG(schur_update(k, k - 1));
         MG(dense_inverse_inplace(h, dc.S[k], dc.nk[k]));
     }
+    for (int k = dc.nlev - 1; k > dc.mid; --k) {  // upper chain, downwards
+        if (k < dc.nlev - 1) MG(schur_update(k, k + 1));
+        MG(dense_inverse_inplace(h, dc.S[k], dc.nk[k]));
+    }
+    if (dc.mid > 0) MG(schur_update(dc.mid, dc.mid - 1));
+    if (dc.mid < dc.nlev - 1) MG(schur_update(dc.mid, dc.mid + 1));
+    MG(dense_inverse_inplace(h, dc.S[dc.mid], dc.nk[dc.mid]));
     if (dc.persist) {   // off-diagonal block rows in the level-set ordering, one contiguous span per level set and side
         LAUNCH(h, direct_pack_ell_kernel, dim3((unsigned)L.n_brows, 2), 128, 0, dc.od_ptr[0], dc.od_pos[0], dc.od_col[0], dc.od_ptr[1],
                dc.od_pos[1], dc.od_col[1], L.vals, b, dc.lev, dc.off, dc.lev_ne, dc.lev_off, dc.ell, dc.ell_col, L.n_brows);
@@ -1040,8 +1110,8 @@ int direct_solve(mg_handle *h, const double *rhs, double *e) {
     const int b = h->b;
     if (dc.persist && h->opt.kernel_variant == 0) {
         DirectSolveArgs a{};
-        a.lv = dc.lvdev;
-        a.nlev = dc.nlev;
+        a.steps = dc.stepdev;
+        a.nsteps = (int)dc.steps.size();
         a.b = b;
         a.ell = dc.ell;
         a.ell_col = dc.ell_col;
@@ -1049,12 +1119,12 @@ int direct_solve(mg_handle *h, const double *rhs, double *e) {
         a.perm = dc.perm;
         a.rhs = rhs;
         a.e = e;
-        a.yb = dc.yb;
-        a.tb = dc.tb;
-        a.bar = dc.bar;
+        a.yb = dc.xchg;
+        a.xb = dc.xchg + L.nvec;
+        a.tb = dc.xchg + 2 * L.nvec;
         a.stages = dc.ds_stages;
         a.tcap = dc.ds_tcap;
-        CU(cudaMemsetAsync(dc.bar, 0, sizeof(unsigned), h->stream));
+        CU(cudaMemsetAsync(dc.xchg, 0xff, sizeof(double) * (size_t)dc.xchg_doubles, h->stream));   // the sentinel: all ones
         void *params[] = {&a};
         ProfPair pp;
         const bool prof = prof_begin(h, pp);
@@ -1064,24 +1134,23 @@ int direct_solve(mg_handle *h, const double *rhs, double *e) {
         count_launch(h);
         return MG_OK;
     }
+    // launch chain: the same steps, one job after the other (jobs of a step are independent)
     LAUNCH_PDL(h, permute_blocks_kernel, grid_for(L.nvec, 256, 1 << 30), 256, 0, rhs, dc.zb, dc.perm, L.n_brows, b, 0);
-    for (int k = 0; k < dc.nlev; ++k) {   // y_k = S_k^-1 (z_k - L_k y_{k-1})
-        const double *zk = dc.zb + dc.voff[k];
-        if (k > 0) {
-            LAUNCH_PDL(h, direct_offdiag_kernel, (dc.nk[k] + 3) / 4, 128, 0, dc.od_ptr[0], dc.od_pos[0], dc.od_col[0], L.vals, b,
-                   dc.voff[k] / b, dc.nk[k], dc.yb, zk, dc.tb, -1.0);
-            zk = dc.tb;
+    for (const auto &st : dc.steps)
+        for (const auto &j : st) {
+            const int k = j.level, nk = dc.nk[k];
+            if (j.phase == 0) {   // y_k = S_k^-1 (z_k - X y)
+                LAUNCH_PDL(h, direct_offdiag_kernel, (nk + 3) / 4, 128, 0, dc.od_ptr[0], dc.od_pos[0], dc.od_col[0], L.vals, b, dc.voff[k] / b,
+                           nk, dc.yb, dc.zb + dc.voff[k], dc.tb, -1.0);
+                LAUNCH_PDL(h, dense_gemv_kernel, (nk + GEMV_ROWS - 1) / GEMV_ROWS, 256, 0, dc.S[k], dc.tb, (const double *)nullptr,
+                           dc.yb + dc.voff[k], nk, nk, 1.0);
+            } else {              // x_k = y_k - S_k^-1 (X x); the solution is built in place in yb
+                LAUNCH_PDL(h, direct_offdiag_kernel, (nk + 3) / 4, 128, 0, dc.od_ptr[1], dc.od_pos[1], dc.od_col[1], L.vals, b, dc.voff[k] / b,
+                           nk, dc.yb, (const double *)nullptr, dc.tb, 1.0);
+                LAUNCH_PDL(h, dense_gemv_kernel, (nk + GEMV_ROWS - 1) / GEMV_ROWS, 256, 0, dc.S[k], dc.tb, dc.yb + dc.voff[k],
+                           dc.yb + dc.voff[k], nk, nk, -1.0);
+            }
         }
-        LAUNCH_PDL(h, dense_gemv_kernel, (dc.nk[k] + GEMV_ROWS - 1) / GEMV_ROWS, 256, 0, dc.S[k], zk, (const double *)nullptr, dc.yb + dc.voff[k],
-               dc.nk[k], dc.nk[k], 1.0);
-    }
-    // x_q = y_q on the last level set, x_k = y_k - S_k^-1 (U_k x_{k+1}); the solution is built in place in yb
-    for (int k = dc.nlev - 2; k >= 0; --k) {
-        LAUNCH_PDL(h, direct_offdiag_kernel, (dc.nk[k] + 3) / 4, 128, 0, dc.od_ptr[1], dc.od_pos[1], dc.od_col[1], L.vals, b,
-               dc.voff[k] / b, dc.nk[k], dc.yb, (const double *)nullptr, dc.tb, 1.0);
-        LAUNCH_PDL(h, dense_gemv_kernel, (dc.nk[k] + GEMV_ROWS - 1) / GEMV_ROWS, 256, 0, dc.S[k], dc.tb, dc.yb + dc.voff[k], dc.yb + dc.voff[k], dc.nk[k],
-               dc.nk[k], -1.0);
-    }
     LAUNCH_PDL(h, permute_blocks_kernel, grid_for(L.nvec, 256, 1 << 30), 256, 0, dc.yb, e, dc.perm, L.n_brows, b, 1);
     CU(cudaGetLastError());
     return MG_OK;
