@@ -16,8 +16,10 @@ once, outside the timed region (it is the paper's lagged "refresh")
 * ``roofline`` = the kernel class with the largest share of the step: algorithmic bytes per launch
   (paper_2506_16676_b200/traffic.py) / its mean CUDA-event duration, measured
   in a short event-bracketed pass right after the timed steps, against MEASURED_PEAKS.json's HBM copy rate.
-* ``cpu_baseline`` = the oracle (oracle/, as it stands) timed on the host cores on a bounded sample and
-  extrapolated by algorithmic bytes to one solve.  A reported baseline, not the target.
+* ``cpu_baseline`` = the oracle (oracle/, as it stands) TIMED on the host cores on bounded units of the same
+  workload (fine-level SpMV, one Chebyshev-PBJ sweep, one V-cycle, coarsest-level PBJ-GMRES iterations); the solve
+  figure is built from those unit times and iteration counts the ORACLE produced (tests/golden/solve_*.json) and is
+  labelled an estimate.  A reported baseline, not the target.
 * N > 1: REPLICAS ONLY -- the path does not shard (north_star: one GPU); N independent solves.
 
 ``--impl reference`` times the oracle alone (no GPU work) and prints the same line with "impl": "reference".
@@ -39,11 +41,11 @@ if ROOT not in sys.path:
 METRIC = "mg_fgmres_solve_time_to_rtol_1e-8"
 UNIT = "s"
 RTOL = 1e-8
-# Extrapolation constants of the oracle arm when no GPU run is at hand (--impl reference runs first, on a fresh
-# box): FGMRES / coarse-GMRES iteration counts of one C1 solve, as measured by this library on a B200 in round 1
-# (the oracle was never run to convergence at this size: hours of CPU time).  Used ONLY to scale a measured
-# oracle GB/s to a solve; never an input or an expected value of any parity test.
-REFERENCE_COUNTS = {"C1": dict(outer_iters=186, coarse_iters=664740), "C0": dict(outer_iters=40, coarse_iters=40000)}
+# Why the N = 1 line is on configs[1] (C1) and not on the largest single-GPU config (C3, 74 GB hierarchy): the driver times
+# 20 complete solves; C3 takes ~150 s per solve in the configs' mode (profiles/r02_configs.md), 20 x 150 s does not fit
+# its window.  `bench.py --workload C3` produces the C3 line.
+WHY_NOT_LARGEST = ("C3 (largest single-GPU config): ~150 s per default-mode solve (profiles/r02_configs.md), x 20 timed steps "
+                   "exceeds the driver's window; bench.py --workload C3 times it")
 
 
 def log(*a):
@@ -112,16 +114,17 @@ class ClockSampler:
 
 
 def measured_traffic(workload: str, level: int, kind: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
-    (profiles/r01_dram_traffic.csv; commands in profiles/r01_tma_kernel.md), or None."""
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures
+    (profiles/r02_dram_traffic.csv, else round 1's; the commands are in the .md beside each), or None."""
     import csv
-    path = os.path.join(ROOT, "profiles", "r01_dram_traffic.csv")
-    if not os.path.exists(path):
-        return None
-    with open(path) as f:
-        for row in csv.DictReader(f):
-            if row["workload"] == workload and int(row["level"]) == level and row["kind"] == kind:
-                return int(row["dram_bytes_per_launch"])
+    for name in ("r02_dram_traffic.csv", "r01_dram_traffic.csv"):
+        path = os.path.join(ROOT, "profiles", name)
+        if not os.path.exists(path):
+            continue
+        with open(path) as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == workload and int(row["level"]) == level and row["kind"] == kind:
+                    return int(row["dram_bytes_per_launch"])
     return None
 
 
@@ -134,9 +137,11 @@ def level_sizes(solver):
     return out
 
 
-def class_bytes(sizes, level, kind, restart_by_level):
+def class_bytes(sizes, level, kind, restart_by_level, direct_bytes: int = 0):
     """Algorithmic bytes of ONE launch of a (level, kind) class (traffic.py)."""
     L = sizes[level]
+    if kind == "direct":    # one direct coarsest-level solve: 2 sum n_k^2 doubles + the off-diagonal blocks (mg_direct_info)
+        return direct_bytes
     if kind in ("spmv", "resid", "sweep", "sweep_nod", "pbj", "restrict", "prolong"):
         return L.by_kind(kind)
     if kind == "cycle":     # one whole restart cycle of the coarsest-level GMRES: m iterations, j = 0..m-1
@@ -146,28 +151,137 @@ def class_bytes(sizes, level, kind, restart_by_level):
 
 
 # ------------------------------------------------------------------------------------------------- oracle arm
-def oracle_sample(w, seconds: float = 15.0):
-    """Time the oracle (as it stands) on a bounded sample of the workload: fine-level block SpMV and PBJ apply,
-    repeated for about ``seconds``.  Returns (GB/s of algorithmic bytes, seconds used, threads, description)."""
-    import numpy as np
+def golden_counts(workload: str):
+    """Iteration counts the ORACLE produced for this workload (tests/golden/solve_*.json, written by
+    tests/golden/make_solve_goldens.py from oracle/ alone): outer FGMRES iterations of a complete solve with the direct
+    coarsest-level solve, and coarsest-level PBJ-GMRES iterations per V-cycle of the configs' own mode.  None if absent."""
+    gdir = os.path.join(ROOT, "tests", "golden")
+    out = {}
+    for key, fname in (("outer", f"solve_{workload}_direct.json"), ("coarse", f"solve_{workload}_default_2its.json"),
+                       ("full", f"solve_{workload}_default.json")):
+        path = os.path.join(gdir, fname)
+        if os.path.exists(path):
+            with open(path) as f:
+                out[key] = json.load(f)
+    if "full" in out:
+        g = out["full"]
+        return dict(outer_iters=g["iters"], coarse_per_cycle=g["coarse_iters_total"] / max(1, g["iters"]),
+                    source=f"tests/golden/solve_{workload}_default.json (complete oracle solve)")
+    if "outer" in out and "coarse" in out:
+        pc = out["coarse"]["coarse_iters_per_cycle"]
+        return dict(outer_iters=out["outer"]["iters"], coarse_per_cycle=sum(pc) / max(1, len(pc)),
+                    source=f"outer count: tests/golden/solve_{workload}_direct.json (complete oracle solve, direct coarse solve); "
+                           f"coarsest-level iterations per V-cycle: tests/golden/solve_{workload}_default_2its.json (oracle, first "
+                           f"{len(pc)} cycles)")
+    return None
+
+
+class OracleUnits:
+    """The oracle's hierarchy of one workload and timers for bounded units of its solve."""
+
+    def __init__(self, w):
+        from oracle import mg as oracle_mg
+        import numpy as np
+        self.mg, self.np, self.w = oracle_mg, np, w
+        t0 = time.perf_counter()
+        # coarse_fixed_sweeps = 0: the V-cycle without its coarsest-level solve (timed separately, per iteration)
+        self.H = oracle_mg.setup(w.row_ptr, w.col_idx, w.vals, w.b, w.n_pol, w.n_phi, w.levels,
+                                 oracle_mg.Options(coarse_mode=1, coarse_fixed_sweeps=0))
+        self.setup_s = time.perf_counter() - t0
+        self.threads = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+        self.rc = np.random.default_rng(7).uniform(-1.0, 1.0, self.H.levels[-1].n)
+
+    def sample(self, coarse_its: int = 40, full: bool = False) -> dict:
+        """One timed sample: seconds of each unit (the oracle exactly as the parity tests call it)."""
+        mg, H, w = self.mg, self.H, self.w
+        L0, Lc = H.levels[0], H.levels[-1]
+        out = {}
+        t0 = time.perf_counter()
+        mg.spmv(L0, w.rhs)
+        out["spmv_fine_s"] = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        mg.vcycle(H, w.rhs)
+        out["vcycle_without_coarsest_s"] = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        _, it, _, _ = mg.fgmres(lambda v: mg.spmv(Lc, v), lambda v: mg.pbj_apply(Lc, v), self.rc, None, 1e-10, 100, coarse_its)
+        out["coarse_gmres_iteration_s"] = (time.perf_counter() - t0) / max(1, it)
+        out["coarse_gmres_iterations_timed"] = it
+        if full:
+            t0 = time.perf_counter()
+            mg.chebyshev(L0, w.rhs, None, 1)
+            out["chebyshev_sweep_fine_s"] = time.perf_counter() - t0
+            H.opt.coarse_fixed_sweeps = 8
+            t0 = time.perf_counter()
+            mg.vcycle(H, w.rhs)
+            out["vcycle_pinned_coarse_mode_s"] = time.perf_counter() - t0
+            H.opt.coarse_fixed_sweeps = 0
+        return out
+
+    @staticmethod
+    def solve_estimate(u: dict, counts: dict) -> float:
+        """Seconds of one solve from measured unit times x oracle-counted iterations (the Gram-Schmidt work of the outer
+        FGMRES is left out: a lower bound)."""
+        per_outer = u["vcycle_without_coarsest_s"] + u["spmv_fine_s"] + counts["coarse_per_cycle"] * u["coarse_gmres_iteration_s"]
+        return counts["outer_iters"] * per_outer
+
+
+def static_config(w, opt: dict, smoother: str = "chebyshev", world: int = 1) -> dict:
+    """The part of ``config`` that names the workload and the method: identical in the CUDA and the reference arm."""
+    return {"workload": w.name, "n_pol": w.n_pol, "n_phi": w.n_phi, "b": w.b, "levels": w.levels, "unknowns": w.n, "nnzb": w.nnzb,
+            "rtol": RTOL,
+            "cycle": f"V({opt['nu_pre']},{opt['nu_post']}) " + ("PBJ-GMRES smoother (the paper's, PAPER.md:95)" if smoother == "gmres"
+                                                                  else "PBJ-Chebyshev"),
+            "coarsest": ("direct (block-tridiagonal Schur inverses)" if opt["coarse_mode"] == 2 else
+                         f"PBJ-GMRES({opt['coarse_restart']}) to {opt['coarse_rtol']:g}"),
+            "fgmres_restart": opt["restart"], "parallelism": "replicas only" if world > 1 else "1 GPU",
+            "why_not_largest": WHY_NOT_LARGEST if w.name == "C1" else None}
+
+
+def reference_arm(args):
+    """The oracle alone on the host cores: each step is one bounded sample of the workload (fine-level SpMV, V-cycle without
+    its coarsest-level solve, 40 coarsest-level PBJ-GMRES iterations); ``value`` is the solve time these unit times give with
+    the oracle's own iteration counts -- an estimate, labelled so; nothing here comes from a GPU run."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_2506_16676_b200.workloads import make_workload
     from oracle import mg as oracle_mg
-    from paper_2506_16676_b200.traffic import LevelSize
-    L = oracle_mg.Level(n_phi=w.n_phi, n_pol=w.n_pol, b=w.b, row_ptr=w.row_ptr, col_idx=w.col_idx, vals=w.vals)
-    L.dinv = oracle_mg.pbj_invert(L)
-    size = LevelSize(n_brows=L.n_brows, nnzb=L.nnzb, b=L.b)
-    x = np.ascontiguousarray(w.rhs)
-    oracle_mg.spmv(L, x)  # page in
-    reps, t0 = 0, time.perf_counter()
-    while True:
-        y = oracle_mg.spmv(L, x)
-        oracle_mg.pbj_apply(L, y)
-        reps += 1
-        if time.perf_counter() - t0 >= seconds or reps >= 5000:
-            break
-    dt = time.perf_counter() - t0
-    gbs = reps * (size.spmv() + size.pbj()) / dt / 1e9
-    threads = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
-    return gbs, dt, threads, f"{reps} x (block SpMV + PBJ apply) on level 0 of {w.name} ({dt:.1f} s of CPU work)"
+    oracle_mg.build()
+    w = make_workload(args.workload)
+    units = OracleUnits(w)
+    counts = golden_counts(args.workload)
+    o = oracle_mg.Options()
+    opt = dict(nu_pre=o.nu_pre, nu_post=o.nu_post, restart=o.restart, coarse_restart=o.coarse_restart, coarse_rtol=o.coarse_rtol,
+               coarse_mode=0)
+    for _ in range(args.warmup):
+        units.sample()
+    vals, samples = [], []
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        u = units.sample()
+        samples.append(u)
+        if counts:
+            vals.append(units.solve_estimate(u, counts))
+    wall = time.perf_counter() - t0
+    value = sum(vals) / len(vals) if vals else None
+    mean = {k: sum(u[k] for u in samples) / len(samples) for k in samples[0]}
+    sample = (f"each step: 1 fine-level block SpMV + 1 V-cycle without its coarsest-level solve + "
+              f"{int(mean['coarse_gmres_iterations_timed'])} coarsest-level PBJ-GMRES iterations of the oracle on {w.name} "
+              f"({wall / max(1, args.steps):.1f} s of CPU work per step); value = ESTIMATE of one solve = oracle-counted iterations x "
+              f"these measured unit times" + (f" [{counts['source']}: {counts['outer_iters']} outer, "
+                                              f"{counts['coarse_per_cycle']:.0f} coarsest-level iterations per V-cycle]" if counts else
+                                              " [no oracle iteration counts for this workload: no estimate]"))
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": (1e3 * value) if value is not None else None,
+            "sample_ms_per_step": 1e3 * wall / max(1, args.steps), "higher_is_better": False,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": static_config(w, opt),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": units.threads, "kind": "oracle", "estimate": True,
+                             "sample": sample, "measured": mean, "oracle_setup_s": units.setup_s},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
 
 
 def orth_bytes(iters, restart, vec_bytes):
@@ -178,65 +292,16 @@ def orth_bytes(iters, restart, vec_bytes):
     return (full * cyc + sum((j + 1) + 8 for j in range(rem))) * vec_bytes
 
 
-def solve_bytes_from_counts(sizes, outer_iters, coarse_iters, opt):
-    """Algorithmic bytes of one solve from iteration counts alone (used to scale the oracle's GB/s)."""
+def solve_bytes_from_counts(sizes, outer_iters, coarse_iters, opt, dram_true: bool = False, direct_bytes: int = 0):
+    """Algorithmic bytes of one solve from its iteration counts.  dram_true: the fused coarse GMRES multiplies by the
+    precomputed A D^-1 and never reads D^-1 (SURVEY's byte model charges it to every coarse iteration).  direct_bytes: bytes of
+    one direct coarsest-level solve (coarse_mode 2)."""
     from paper_2506_16676_b200.traffic import vcycle_bytes
     L0, Lc = sizes[0], sizes[-1]
-    outer = outer_iters * (vcycle_bytes(sizes, opt["nu_pre"], opt["nu_post"]) + L0.spmv()) + \
+    outer = outer_iters * (vcycle_bytes(sizes, opt["nu_pre"], opt["nu_post"]) + L0.spmv() + direct_bytes) + \
         orth_bytes(outer_iters, opt["restart"], L0.vec_bytes)
-    coarse = coarse_iters * (Lc.spmv() + Lc.pbj()) + orth_bytes(coarse_iters, opt["coarse_restart"], Lc.vec_bytes)
+    coarse = coarse_iters * (Lc.spmv() + (0 if dram_true else Lc.pbj())) + orth_bytes(coarse_iters, opt["coarse_restart"], Lc.vec_bytes)
     return outer + coarse
-
-
-def oracle_level_sizes(w):
-    """Level sizes of the hierarchy from the closed-form Galerkin pattern (no numerics): level l+1 has the prism
-    stencil of level l's node graph over min(3, n_phi) planes."""
-    import numpy as np
-    from paper_2506_16676_b200.traffic import LevelSize
-    sizes = [LevelSize(n_brows=w.n_brows, nnzb=w.nnzb, b=w.b)]
-    edges = w.adj_w[0]
-    deg = np.bincount(edges.ravel(), minlength=w.n_pol) + 1   # in-plane blocks per row incl. self
-    n_phi = w.n_phi
-    for _ in range(1, w.levels):
-        n_phi //= 2
-        sizes.append(LevelSize(n_brows=n_phi * w.n_pol, nnzb=int(deg.sum()) * n_phi * min(3, n_phi), b=w.b))
-    return sizes
-
-
-def reference_arm(args):
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
-        return 0
-    from paper_2506_16676_b200.workloads import make_workload
-    from oracle import mg as oracle_mg
-    oracle_mg.build()
-    w = make_workload(args.workload)
-    sizes = oracle_level_sizes(w)
-    opt = dict(nu_pre=2, nu_post=2, restart=100, coarse_restart=100)
-    counts = REFERENCE_COUNTS.get(args.workload, REFERENCE_COUNTS["C1"])
-    total_bytes = solve_bytes_from_counts(sizes, counts["outer_iters"], counts["coarse_iters"], opt)
-    per_step = max(0.05, min(args.cpu_seconds, 150.0 / max(1, args.steps + args.warmup)))
-    for _ in range(args.warmup):
-        oracle_sample(w, per_step)
-    vals, desc, threads = [], "", 1
-    t0 = time.perf_counter()
-    for _ in range(args.steps):
-        gbs, dt, threads, desc = oracle_sample(w, per_step)
-        vals.append(total_bytes / 1e9 / gbs)
-    wall = time.perf_counter() - t0
-    value = sum(vals) / len(vals)
-    sample = (f"each step: {desc}; measured oracle rate scaled by algorithmic bytes to one solve of "
-              f"{counts['outer_iters']} outer / {counts['coarse_iters']} coarsest-level iterations (counts measured by the "
-              f"CUDA library in round 1; the oracle is not run to convergence at this size)")
-    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": 1e3 * wall / max(1, args.steps), "higher_is_better": False,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": args.workload, "rtol": RTOL, "extrapolated": True},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
-            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-            "gpu_launches": 0}
-    print(json.dumps(line), flush=True)
-    return 0
 
 
 # ------------------------------------------------------------------------------------------------- CUDA arm
@@ -330,6 +395,8 @@ def cuda_arm(args):
     peak, peak_src = measured_peaks()
     roof, detail, cpu, vcycle_roof, direct = None, [], None, None, None
     if rank == 0:
+        dinfo = s.direct_info() if opt["coarse_mode"] == 2 else None
+        direct_bytes = dinfo["bytes_per_solve"] if dinfo else 0
         s.update_options(maxit=min(opt["maxit"], 2))
         s.profile_reset()
         s.profile_enable(True)
@@ -338,16 +405,14 @@ def cuda_arm(args):
         timed = s.profile_get()
         s.update_options(maxit=opt["maxit"])
         restart_by_level = {s.levels - 1: opt["coarse_restart"]}
-        step_ms_model = 0.0
         for (level, kind), c in counts.items():
             t = timed.get((level, kind))
             if not t or not t["timed"]:
                 continue
             mean_ms = t["ms"] / t["timed"]
             per_step_launches = c["launches"] / args.steps
-            nbytes = class_bytes(sizes, level, kind, restart_by_level)
+            nbytes = class_bytes(sizes, level, kind, restart_by_level, direct_bytes)
             share_ms = per_step_launches * mean_ms
-            step_ms_model += share_ms
             detail.append({"level": level, "kind": kind, "launches_per_step": per_step_launches, "mean_us": 1e3 * mean_ms,
                            "bytes_per_launch": nbytes, "GBps": (nbytes / mean_ms / 1e6) if nbytes else None,
                            "frac": (nbytes / mean_ms / 1e6 / peak) if nbytes else None, "ms_per_step": share_ms})
@@ -356,7 +421,9 @@ def cuda_arm(args):
             d["share_of_step"] = d["ms_per_step"] / (1e3 * t_dev)
         top = next((d for d in detail if d["bytes_per_launch"]), None)
         if top:
-            roof = {"bound": "hbm", "kernel": f"bsr kernel, kind {top['kind']}, level {top['level']}", "achieved": top["GBps"],
+            what = ("direct coarsest-level solve (direct_solve_persistent_kernel)" if top["kind"] == "direct" else
+                    f"bsr kernel, kind {top['kind']}, level {top['level']}")
+            roof = {"bound": "hbm", "kernel": what, "achieved": top["GBps"],
                     "peak": peak, "unit": "GB/s", "frac": top["frac"],
                     "traffic": measured_traffic(w.name, top["level"], top["kind"]), "peak_source": peak_src,
                     "bytes_per_launch": top["bytes_per_launch"], "mean_us": top["mean_us"],
@@ -379,14 +446,21 @@ def cuda_arm(args):
         s.update_options(coarse_mode=opt["coarse_mode"])
         vc_ms = v0.elapsed_time(v1) / 5
         vc_bytes = vcycle_bytes(sizes, opt["nu_pre"], opt["nu_post"], coarse_sweeps=s.opt.coarse_fixed_sweeps)
-        solve_bytes = solve_bytes_from_counts(sizes, info["iters"], info["coarse_iters_total"], opt)
+        solve_bytes = solve_bytes_from_counts(sizes, info["iters"], info["coarse_iters_total"], opt, direct_bytes=direct_bytes)
+        solve_bytes_dram = solve_bytes_from_counts(sizes, info["iters"], info["coarse_iters_total"], opt, dram_true=True,
+                                                   direct_bytes=direct_bytes)
         vcycle_roof = None if args.smoother == "gmres" else {   # the byte model below is the Chebyshev cycle's
             "pinned_coarse_mode": {"ms": vc_ms, "bytes": vc_bytes, "GBps": vc_bytes / vc_ms / 1e6,
                                    "frac_of_measured_peak": vc_bytes / vc_ms / 1e6 / peak, "frac_of_8TBs_nominal": vc_bytes / vc_ms / 1e6 / 8000.0},
             "complete_outer_iteration": {"ms": 1e3 * t_dev / max(1, info["iters"]), "bytes": solve_bytes / max(1, info["iters"]),
                                          "GBps": solve_bytes / t_dev / 1e9, "frac_of_measured_peak": solve_bytes / t_dev / 1e9 / peak,
                                          "frac_of_8TBs_nominal": solve_bytes / t_dev / 1e9 / 8000.0,
-                                         "coarse_steps_per_cycle": info["coarse_iters_total"] / max(1, info["iters"])}}
+                                         "coarse_steps_per_cycle": info["coarse_iters_total"] / max(1, info["iters"]),
+                                         "byte_model": "SURVEY 8d: every coarsest-level iteration charged A + D^-1"},
+            # what DRAM really moves: the fused coarse GMRES multiplies by the precomputed A D^-1 and never reads D^-1
+            "complete_outer_iteration_dram_true": {"bytes": solve_bytes_dram / max(1, info["iters"]), "GBps": solve_bytes_dram / t_dev / 1e9,
+                                                   "frac_of_measured_peak": solve_bytes_dram / t_dev / 1e9 / peak,
+                                                   "frac_of_8TBs_nominal": solve_bytes_dram / t_dev / 1e9 / 8000.0}}
         # ---- the same solve with the paper's kind of coarsest-level solver (direct, NEXT-2): reported beside the metric,
         # which keeps the configs' PBJ-GMRES coarse solve
         direct = None
@@ -398,43 +472,57 @@ def cuda_arm(args):
                 torch.cuda.synchronize()
                 first_s = time.perf_counter() - t0d
                 _, info_d = s.solve_host(rhs_h, x_h, rtol=RTOL)
+                di = s.direct_info()
+                # the coarsest-level solve alone: CUDA events around 20 back-to-back calls
+                rc = torch.rand(s.n(s.levels - 1), dtype=torch.float64, device=dev) * 2 - 1
+                ec = s.new(s.levels - 1)
+                for _ in range(3):
+                    s.coarse_solve(rc, ec)
+                c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                c0.record()
+                for _ in range(20):
+                    s.coarse_solve(rc, ec)
+                c1.record()
+                torch.cuda.synchronize()
+                cs_ms = c0.elapsed_time(c1) / 20
                 direct = {"value": info_d["solve_ms"] / 1e3, "unit": UNIT, "outer_iters": info_d["iters"], "rel_res": info_d["rel_res"],
                           "converged": info_d["converged"], "factorisation_s": max(0.0, first_s - info_d["solve_ms"] / 1e3),
+                          "coarse_solve": {"us": 1e3 * cs_ms, "bytes": di["bytes_per_solve"], "GBps": di["bytes_per_solve"] / cs_ms / 1e6,
+                                           "frac_of_measured_peak": di["bytes_per_solve"] / cs_ms / 1e6 / peak,
+                                           "level_sets": di["level_sets"], "dense_GB": di["dense_bytes"] / 1e9,
+                                           "persistent_kernel": di["persistent"]},
                           "what": "mg_options.coarse_mode = 2: block-tridiagonal direct solve of the coarsest level "
                                   "(the paper solves its coarsest level by LU, PAPER.md:374-381); not the metric's configuration"}
             except Exception as exc:   # e.g. not enough memory for the dense blocks
                 direct = {"unavailable": str(exc)}
             finally:
                 s.update_options(coarse_mode=opt["coarse_mode"])
-        # ---- oracle timed beside it (rank 0, N = 1 only)
+        # ---- oracle timed beside it (rank 0, N = 1 only): bounded units of the same workload on the host cores
         if world == 1 and not args.no_cpu_baseline:
-            gbs, dt, threads, desc = oracle_sample(w, args.cpu_seconds)
-            total_bytes = sum(c["launches"] / args.steps * class_bytes(sizes, level, kind, restart_by_level)
-                              for (level, kind), c in counts.items())
-            # orthogonalisation launches carry no per-launch size: their traffic follows from the iteration counts
-            total_bytes += orth_bytes(info["iters"], opt["restart"], sizes[0].vec_bytes)
-            if not any(kind == "cycle" for (_, kind) in counts):
-                total_bytes += orth_bytes(info["coarse_iters_total"], opt["coarse_restart"], sizes[-1].vec_bytes)
-            cpu = {"value": total_bytes / 1e9 / gbs, "unit": UNIT, "cores": threads, "kind": "oracle",
-                   "oracle_GBps": gbs,
-                   "sample": f"{desc}; its algorithmic GB/s scaled to the {total_bytes / 1e9:.0f} GB of algorithmic "
-                             f"traffic of one solve ({info['iters']} outer, {info['coarse_iters_total']} coarsest-level iterations)"}
+            units = OracleUnits(w)
+            u = units.sample(full=True)
+            gc_ = golden_counts(w.name) if opt["coarse_mode"] == 0 and args.smoother == "chebyshev" and args.levels <= 0 else None
+            est = units.solve_estimate(u, gc_) if gc_ else None
+            cpu = {"value": est, "unit": UNIT, "cores": units.threads, "kind": "oracle", "estimate": True, "measured": u,
+                   "oracle_setup_s": units.setup_s,
+                   "sample": (f"oracle units timed on {w.name}: fine-level block SpMV, one Chebyshev-PBJ sweep, one V-cycle (pinned "
+                              f"coarse mode and without the coarsest level), {u['coarse_gmres_iterations_timed']} coarsest-level "
+                              f"PBJ-GMRES iterations; value = ESTIMATE of one solve = oracle-counted iterations x these unit times"
+                              + (f" [{gc_['source']}: {gc_['outer_iters']} outer, {gc_['coarse_per_cycle']:.0f} coarsest-level "
+                                 f"iterations per V-cycle]" if gc_ else " [no oracle iteration counts for this configuration: no estimate]"))}
 
     if rank == 0:
+        cfg = static_config(w, opt, args.smoother, world)
+        cfg["l2"] = ("inputs larger than L2 (every level's matrix >= 0.5 GB vs 126 MB L2)" if sizes[-1].matrix_bytes > 2.6e8
+                     else "coarsest level fits L2: not an HBM-roofline workload")
+        cfg["warmup_steps"] = (f"{args.warmup} x the first {args.warmup_outer} outer iterations of the same solve"
+                               if args.warmup_outer > 0 and args.max_outer <= 0 else f"{args.warmup} x complete solves")
         line = {"metric": METRIC, "value": t_dev, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": 1e3 * t_dev, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
-                "dtype": "f64", "data": "synthetic",
-                "config": {"workload": w.name, "n_pol": w.n_pol, "n_phi": w.n_phi, "b": w.b, "levels": w.levels,
-                           "unknowns": n, "nnzb": w.nnzb, "rtol": RTOL, "cycle": f"V({opt['nu_pre']},{opt['nu_post']}) " + ("PBJ-GMRES smoother (the paper's, PAPER.md:95)" if args.smoother == "gmres" else "PBJ-Chebyshev"),
-                           "coarsest": ("direct (block-tridiagonal Schur inverses)" if opt["coarse_mode"] == 2 else
-                                        f"PBJ-GMRES({opt['coarse_restart']}) to {opt['coarse_rtol']:g}"), "fgmres_restart": opt["restart"],
-                           "parallelism": "replicas only" if world > 1 else "1 GPU", "setup_s": setup_s, "refresh_s": refresh_s,
-                           "l2": "inputs larger than L2 (every level's matrix >= 0.5 GB vs 126 MB L2)" if sizes[-1].matrix_bytes > 2.6e8
-                           else "coarsest level fits L2: not an HBM-roofline workload",
-                           "warmup_steps": (f"{args.warmup} x the first {args.warmup_outer} outer iterations of the same solve"
-                                            if args.warmup_outer > 0 and args.max_outer <= 0 else f"{args.warmup} x complete solves"),
-                           "outer_iters": info["iters"], "coarse_iters": info["coarse_iters_total"], "rel_res": info["rel_res"],
-                           "max_abs_x": x_dev_check},
+                "dtype": "f64", "data": "synthetic", "config": cfg,
+                "solve": {"outer_iters": info["iters"], "coarse_iters": info["coarse_iters_total"], "rel_res": info["rel_res"],
+                          "max_abs_x": x_dev_check, "setup_s": setup_s, "refresh_s": refresh_s,
+                          "hierarchy_GB": s.device_bytes() / 1e9, "fine_matrix_GB": va.numel() * 8 / 1e9},
                 "e2e": {"value": t_e2e, "unit": UNIT, "h2d_bytes_per_step": 8 * n, "d2h_bytes_per_step": 8 * n},
                 "gpu_launches": launches, "clocks": clocks, "roofline": roof, "vcycle_roofline": vcycle_roof, "direct_coarse_solve": direct, "cpu_baseline": cpu,
                 "throughput": {"value": world / t_dev, "unit": "solves/s"}, "truncated": args.max_outer > 0,
@@ -468,7 +556,6 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
     ap.add_argument("--workload", default="C1", help="C1 (the metric's config, default); C0, C2-16/32/64, C3, C3b for other configs")
-    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="CPU time of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-direct", action="store_true", help="skip the extra solve with the direct coarsest-level solver")
     ap.add_argument("--max-outer", type=int, default=0,

@@ -18,8 +18,11 @@
 //     9-double stride are bank-conflict free, the 4 partial sums of a row meet by two warp shuffles, blocks are
 //     added in stored order (deterministic).  After the last read of a stage each consumer warp arrives on the
 //     stage's "empty" mbarrier, which hands it back to the producer;
-//   * the row epilogue is the fused part: residual, x update, z = Dinv_I r_I (Dinv_I prefetched into registers at
-//     row start, 9 doubles per thread), Chebyshev direction update -- kernels_bsr.cuh documents the modes.
+//   * the row epilogue is the fused part: residual, x update, z = Dinv_I r_I, Chebyshev direction update --
+//     kernels_bsr.cuh documents the modes.  In a sweep Dinv_I rides in the SAME ring: the producer appends it to the
+//     stream after the last block of every owned row, and the consumers multiply it by r_I exactly as they multiply a
+//     block of A by x_J (round 1 fetched it with 72-byte per-thread loads into registers: the sweep then ran 4-5 %
+//     below the SpMV pass in GB/s).
 //
 // PBJ apply alone is the same kernel on the implicit block-diagonal matrix `dinv` (row I = block I = column I).
 #pragma once
@@ -40,10 +43,10 @@ struct TmaCfg {
     static constexpr int NG = 4;                      // consumer groups per CTA (3: -8 %, 5: no gain)
     static constexpr int STAGES = 20;
     static constexpr int THREADS = NG * GROUP + 32;   // + 1 producer warp
-    static constexpr int VECPAD = 40;
+    static constexpr int VECPAD = 40;                 // per group and row parity: the new residual r_I for the Dinv product
     static constexpr unsigned POLL_NS = 1000;         // sleep between polls of the producer's per-stage round counters
     static constexpr unsigned SWEEP_MBAR_NS = 100;    // back-off of the full-barrier wait in the fused sweep
-    static constexpr size_t SMEM = sizeof(double) * ((size_t)STAGES * (BB + B) + NG * VECPAD) + sizeof(uint64_t) * (3 * STAGES);
+    static constexpr size_t SMEM = sizeof(double) * ((size_t)STAGES * (BB + B) + 2 * NG * VECPAD) + sizeof(uint64_t) * (3 * STAGES);
 };
 
 // extra arguments of the TMA kernel (the common ones are BsrArgs)
@@ -162,7 +165,7 @@ __global__ void __launch_bounds__(TmaCfg::THREADS, 1) bsr_tma_kernel(const BsrAr
     double *sA = reinterpret_cast<double *>(smem_raw);
     double *sX = sA + (size_t)C::STAGES * BB;
     double *sVec = sX + C::STAGES * B;
-    uint64_t *full = reinterpret_cast<uint64_t *>(sVec + C::NG * C::VECPAD);
+    uint64_t *full = reinterpret_cast<uint64_t *>(sVec + 2 * C::NG * C::VECPAD);
     uint64_t *empty = full + C::STAGES;
     // round_of[s] = number of rounds for which stage s has been issued.  A consumer group may be more than one ring
     // round ahead of the stage it wants next (its row starts >= STAGES blocks after the oldest block still in flight);
@@ -204,24 +207,44 @@ __global__ void __launch_bounds__(TmaCfg::THREADS, 1) bsr_tma_kernel(const BsrAr
     if (warp == C::NG * C::GWARPS) {
         // ------------------------------------------------------------------ producer warp: stream blocks P0..P1
         const uint64_t pol = policy_evict_first();
-        const int total = (int)(P1 - P0);
-        // Every lane < PL issues its own block: the waits on the stages' "empty" barriers and the issue latencies
+        // Sweep with the Dinv product: the stream is [head fragment blocks] then, per owned row I, its blocks inside
+        // [P0, P1) followed by Dinv_I; ring counter of row I's first block: f(I) = row_ptr[I] - P0 + (I - R0).
+        const bool with_dinv = (a.mode == MODE_SWEEP) && (a.flags & F_NEED_D);
+        const int total = (int)(P1 - P0) + (with_dinv ? (int)(R1 - R0) : 0);
+        // Every lane < PL issues its own stage: the waits on the stages' "empty" barriers and the issue latencies
         // overlap (one issuing thread was the pacing element of the whole kernel: +5-7 % on levels 1-3).  round_of[s]
         // tells the consumers that stage s has been (re)issued for round k, see above.
         constexpr int PL = 16;
+        int64_t Icur = R0;   // row cursor of this lane (with_dinv): largest owned row with f(I) <= i so far
         for (int base = 0; base < total; base += PL) {
             const int i = base + lane;
             if (lane < PL && i < total) {
-                const int j = diag ? (int)(P0 + i) : __ldg(a.col_idx + P0 + i);
+                int64_t pblk = P0 + i;   // block to copy, or -1: Dinv of row Icur
+                if (with_dinv) {
+                    const int64_t fR0 = __ldg(a.row_ptr + R0) - P0;
+                    if (i >= fR0 && R1 > R0) {
+                        while (Icur + 1 < R1 && __ldg(a.row_ptr + Icur + 1) - P0 + (Icur + 1 - R0) <= i) ++Icur;
+                        const int64_t rp = __ldg(a.row_ptr + Icur);
+                        const int64_t o = i - (rp - P0 + (Icur - R0));
+                        const int64_t nblk = min(__ldg(a.row_ptr + Icur + 1), P1) - rp;
+                        pblk = o < nblk ? rp + o : -1;
+                    }
+                }
                 const int s = i % C::STAGES, k = i / C::STAGES;
                 mbar_wait(&empty[s], ((uint32_t)k & 1u) ^ 1u);
                 round_of[s] = k + 1;
-                mbar_expect_tx(&full[s], (uint32_t)((BB + B) * sizeof(double)));
-                // the matrix stream is read once per launch: evict-first keeps the vectors, the Krylov basis and (on small
-                // levels) Dinv resident in the 126 MB L2; Dinv itself (PBJ apply) is loaded with the default policy
-                if (diag) bulk_g2s(sA + (size_t)s * BB, stream + (size_t)(P0 + i) * BB, BB * sizeof(double), &full[s]);
-                else bulk_g2s_hint(sA + (size_t)s * BB, stream + (size_t)(P0 + i) * BB, BB * sizeof(double), &full[s], pol);
-                bulk_g2s(sX + s * B, xsrc + (size_t)j * B, B * sizeof(double), &full[s]);
+                if (pblk < 0) {   // Dinv_I: multiplied by the residual the consumers hold, no x block
+                    mbar_expect_tx(&full[s], (uint32_t)(BB * sizeof(double)));
+                    bulk_g2s(sA + (size_t)s * BB, a.dinv + (size_t)Icur * BB, BB * sizeof(double), &full[s]);
+                } else {
+                    const int j = diag ? (int)pblk : __ldg(a.col_idx + pblk);
+                    mbar_expect_tx(&full[s], (uint32_t)((BB + B) * sizeof(double)));
+                    // the matrix stream is read once per launch: evict-first keeps the vectors, the Krylov basis and (on small
+                    // levels) Dinv resident in the 126 MB L2; Dinv itself is loaded with the default policy
+                    if (diag) bulk_g2s(sA + (size_t)s * BB, stream + (size_t)pblk * BB, BB * sizeof(double), &full[s]);
+                    else bulk_g2s_hint(sA + (size_t)s * BB, stream + (size_t)pblk * BB, BB * sizeof(double), &full[s], pol);
+                    bulk_g2s(sX + s * B, xsrc + (size_t)j * B, B * sizeof(double), &full[s]);
+                }
             }
             __syncwarp();
         }
@@ -237,7 +260,7 @@ __global__ void __launch_bounds__(TmaCfg::THREADS, 1) bsr_tma_kernel(const BsrAr
     const bool sweep = (a.mode == MODE_SWEEP);
     const bool need_d = sweep && (flags & F_NEED_D);
     const bool touch_x = (flags & (F_UPD_X | F_SET_X | F_FINAL_X)) != 0;
-    double *vec = sVec + g * C::VECPAD;
+    double *vecbase = sVec + 2 * g * C::VECPAD;
     double inv_scale = 1.0;
     const bool spmv_scaled = (a.mode == MODE_SPMV) && ex.scale_div != nullptr;
     if (spmv_scaled) inv_scale = 1.0 / *ex.scale_div;
@@ -265,20 +288,13 @@ __global__ void __launch_bounds__(TmaCfg::THREADS, 1) bsr_tma_kernel(const BsrAr
         if (open) p1 = P1;
         const size_t gi = (size_t)I * B + r;
         double rin_v = 0.0, dold = 0.0, xold = 0.0;
-        double dreg[C::SEGL];
-#pragma unroll
-        for (int c = 0; c < C::SEGL; ++c) dreg[c] = 0.0;
         if (active && !frag) {
             if (a.mode == MODE_RESID || sweep) rin_v = a.rin[gi];
             if (sweep || (spmv_scaled && ex.vout != nullptr)) dold = a.vin[gi];
             if (touch_x && !(flags & F_SET_X)) xold = a.x[gi];
-            if (need_d) {
-                const double *dp = a.dinv + (size_t)I * BB + C::SEGL * t;
-#pragma unroll
-                for (int c = 0; c < C::SEGL; ++c) dreg[c] = __ldg(dp + c);
-            }
         }
-        int n = (int)(p0 - P0);
+        // ring counter of the item's first block (with Dinv stages in the stream: one per owned row before this one)
+        int n = (int)(p0 - P0) + ((need_d && !frag) ? (int)(I - R0) : 0);
         int s = n % C::STAGES;
         uint32_t ph = (uint32_t)(n / C::STAGES) & 1u;
         double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0;
@@ -358,16 +374,33 @@ __global__ void __launch_bounds__(TmaCfg::THREADS, 1) bsr_tma_kernel(const BsrAr
                     else if (flags & F_UPD_X) a.x[gi] = xold + dold;
                 }
             } else {
+                // z = Dinv_I r': Dinv_I is the next stage of the ring (s, ph, n already point at it); r' goes through a
+                // per-group buffer, double-buffered by row parity so that one group barrier per row suffices
+                double *vec = vecbase + (((it - g) / C::NG) & 1) * C::VECPAD;
                 if (writer) vec[r] = rnew;
                 group_bar(g);
+                while (round_of[s] <= n / C::STAGES) __nanosleep(C::POLL_NS);
+                mbar_wait_backoff(&full[s], ph, mbar_ns);
                 double z = 0.0;
                 if (active) {
-#pragma unroll
-                    for (int c = 0; c < C::SEGL; ++c) z = fma(dreg[c], vec[C::SEGL * h + c], z);
+                    const double *D = sA + (size_t)s * BB + C::SEGL * t;
+                    const double *vs = vec + C::SEGL * h;
+                    double z0 = 0.0, z1 = 0.0, z2 = 0.0;
+                    z0 = fma(D[0], vs[0], z0);
+                    z1 = fma(D[1], vs[1], z1);
+                    z2 = fma(D[2], vs[2], z2);
+                    z0 = fma(D[3], vs[3], z0);
+                    z1 = fma(D[4], vs[4], z1);
+                    z2 = fma(D[5], vs[5], z2);
+                    z0 = fma(D[6], vs[6], z0);
+                    z1 = fma(D[7], vs[7], z1);
+                    z2 = fma(D[8], vs[8], z2);
+                    z = (z0 + z1) + z2;
                 }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&empty[s]);
                 z += __shfl_xor_sync(0xffffffffu, z, 1);
                 z += __shfl_xor_sync(0xffffffffu, z, 2);
-                group_bar(g);
                 if (writer) {
                     double dnew = a.c_z * z;
                     if (a.c_d != 0.0) dnew = fma(a.c_d, dold, dnew);

@@ -44,6 +44,10 @@ CASES = {
     # config 3's recipe (non-axisymmetric, beta = 0.5, sigma = 1e-4, delta = 0.15, 32 -> 2 planes) on a reduced mesh
     "C3r_default": ("C3", dict(mesh=(4, 16)), dict(coarse_mode=0)),
     "C3r_direct": ("C3", dict(mesh=(4, 16)), dict(coarse_mode=2)),
+    # config 1 in the configs' own mode, cut after 2 outer iterations (a complete default-mode solve is ~6e5 coarsest-level
+    # GMRES steps of 0.56 GB each: days of CPU time): the residual history of the first iterations and the oracle's
+    # coarsest-level iteration count per V-cycle, which bench.py's cpu_baseline estimate uses
+    "C1_default_2its": ("C1", {}, dict(coarse_mode=0, maxit=2)),
 }
 
 
@@ -55,8 +59,20 @@ def run_case(case: str, rtol: float = 1e-8) -> dict:
     w = make_workload(name, **over)
     H = mg.setup(w.row_ptr, w.col_idx, w.vals, w.b, w.n_pol, w.n_phi, w.levels, mg.Options(**opt))
     t_setup = time.perf_counter() - t0
+    per_cycle = []
+    inner = mg.coarse_solve
+
+    def counting_coarse_solve(Hh, rhs):   # record the coarsest-level iteration count of every V-cycle
+        e = inner(Hh, rhs)
+        per_cycle.append(int(Hh.coarse_iters_last))
+        return e
+
+    mg.coarse_solve = counting_coarse_solve
     t0 = time.perf_counter()
-    x, iters, converged, hist = mg.solve(H, w.rhs, rtol)
+    try:
+        x, iters, converged, hist = mg.solve(H, w.rhs, rtol)
+    finally:
+        mg.coarse_solve = inner
     t_solve = time.perf_counter() - t0
     import numpy as np
     true_rel = float(np.linalg.norm(w.rhs - mg.spmv(H.levels[0], x)) / np.linalg.norm(w.rhs))
@@ -74,6 +90,7 @@ def run_case(case: str, rtol: float = 1e-8) -> dict:
         "iters": int(iters),
         "converged": bool(converged),
         "coarse_iters_total": int(H.coarse_iters_total),
+        "coarse_iters_per_cycle": per_cycle if len(per_cycle) <= 16 else per_cycle[:8] + per_cycle[-8:],
         "true_rel_res": true_rel,
         "rho_est": [float(L.rho_est) for L in H.levels],
         "hist": [float(h) for h in hist],
