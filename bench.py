@@ -254,11 +254,11 @@ def reference_arm(args):
     opt = dict(nu_pre=o.nu_pre, nu_post=o.nu_post, restart=o.restart, coarse_restart=o.coarse_restart, coarse_rtol=o.coarse_rtol,
                coarse_mode=0)
     for _ in range(args.warmup):
-        units.sample()
+        units.sample(args.ref_coarse_its)
     vals, samples = [], []
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        u = units.sample()
+        u = units.sample(args.ref_coarse_its)
         samples.append(u)
         if counts:
             vals.append(units.solve_estimate(u, counts))
@@ -500,7 +500,7 @@ def cuda_arm(args):
         # ---- oracle timed beside it (rank 0, N = 1 only): bounded units of the same workload on the host cores
         if world == 1 and not args.no_cpu_baseline:
             units = OracleUnits(w)
-            u = units.sample(full=True)
+            u = units.sample(args.ref_coarse_its, full=True)
             gc_ = golden_counts(w.name) if opt["coarse_mode"] == 0 and args.smoother == "chebyshev" and args.levels <= 0 else None
             est = units.solve_estimate(u, gc_) if gc_ else None
             cpu = {"value": est, "unit": UNIT, "cores": units.threads, "kind": "oracle", "estimate": True, "measured": u,
@@ -557,6 +557,8 @@ def main():
     ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
     ap.add_argument("--workload", default="C1", help="C1 (the metric's config, default); C0, C2-16/32/64, C3, C3b for other configs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ref-coarse-its", type=int, default=40,
+                    help="coarsest-level PBJ-GMRES iterations in one timed oracle sample (cpu_baseline / --impl reference)")
     ap.add_argument("--no-direct", action="store_true", help="skip the extra solve with the direct coarsest-level solver")
     ap.add_argument("--max-outer", type=int, default=0,
                     help="profiling aid (ncu launch lists): cap the outer FGMRES iterations of every solve; the line is then "

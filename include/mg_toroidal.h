@@ -74,7 +74,6 @@ typedef struct mg_options {
     int coarse_restart, coarse_maxit, coarse_fixed_sweeps; /* defaults 100, 20000, 8 (restart: DESIGN.md Q9) */
     int restart, maxit;      /* outer FGMRES restart length and iteration cap; defaults 100, 400
                                 (paper: 200 / 200) */
-    int block_layout;        /* 0: row-major b x b blocks (only layout supported) */
     int use_graphs;          /* 1 (default): the coarse GMRES restart cycle is replayed as a CUDA graph */
     int kernel_variant;      /* launch mechanics only (same arithmetic up to summation order): 0 (default) the
                                 persistent TMA-ring block-CSR kernel where it exists (b = 36), 1 the one-CTA-per-row
@@ -112,7 +111,9 @@ size_t mg_sizeof_solve_info(void);
  * (Gauss-Jordan, partial pivoting), estimate rho(D^-1 A) by eig_iters power iterations from the start
  * vector v0[g] = ((g*2654435761) mod 2^32)/2^32 - 1/2, and form A_{l+1} = P^T A_l P.
  *   row_ptr  int64[n_brows+1], col_idx int32[nnzb] (ascending within a row), vals double[nnzb*b*b]
- *   (row-major blocks): the fine matrix, DEVICE pointers, borrowed until mg_destroy.
+ *   (ROW-MAJOR b x b blocks, the only layout: the fine matrix is borrowed, never copied, so a column-major input
+ *   (SURVEY 8b proposed a flag) would need a transposed copy of up to 55 GB; the caller transposes instead):
+ *   the fine matrix, DEVICE pointers, borrowed until mg_destroy.
  *   n_brows = n_pol*n_phi; levels >= 1; n_phi divisible by 2^(levels-1); 1 <= b <= 64.
  *   levels == 1 is legal: mg_vcycle is then the coarsest-level solve on the fine matrix.
  *   opt may be NULL (defaults).  cuda_stream is a cudaStream_t (NULL = legacy default stream).
@@ -121,7 +122,7 @@ int mg_setup(mg_handle **h, const int64_t *row_ptr, const int32_t *col_idx, cons
              int n_phi, int levels, const mg_options *opt, void *cuda_stream);
 
 /* Replace the solve-phase options (nu, Chebyshev interval factors, coarse_*, restart, maxit) without
- * rebuilding the hierarchy; alloc/free/eig_iters/block_layout are ignored. */
+ * rebuilding the hierarchy; alloc/free/eig_iters are ignored. */
 int mg_update_options(mg_handle *h, const mg_options *opt);
 
 /* Lagged preconditioner ("one new Jacobian per time step ... the preconditioner

@@ -23,7 +23,7 @@ class mg_options(C.Structure):
     _fields_ = [("nu_pre", C.c_int), ("nu_post", C.c_int), ("cheb_lo", C.c_double), ("cheb_hi", C.c_double),
                 ("eig_iters", C.c_int), ("coarse_mode", C.c_int), ("coarse_rtol", C.c_double),
                 ("coarse_restart", C.c_int), ("coarse_maxit", C.c_int), ("coarse_fixed_sweeps", C.c_int),
-                ("restart", C.c_int), ("maxit", C.c_int), ("block_layout", C.c_int), ("use_graphs", C.c_int), ("kernel_variant", C.c_int), ("smoother", C.c_int), ("orth_eta", C.c_double),
+                ("restart", C.c_int), ("maxit", C.c_int), ("use_graphs", C.c_int), ("kernel_variant", C.c_int), ("smoother", C.c_int), ("orth_eta", C.c_double),
                 ("alloc", ALLOC_FN), ("free", FREE_FN), ("alloc_ctx", C.c_void_p)]
 
 

@@ -1520,7 +1520,6 @@ int mg_options_default(mg_options *o) {
     o->coarse_fixed_sweeps = 8;
     o->restart = 100;
     o->maxit = 400;
-    o->block_layout = 0;
     o->use_graphs = 1;
     o->kernel_variant = 0;
     o->smoother = 0;
@@ -1536,7 +1535,7 @@ static int validate_options(const mg_options &o) {
     if (!(o.cheb_lo > 0.0) || !(o.cheb_hi > o.cheb_lo)) return MG_EINVAL;
     if (o.coarse_mode < 0 || o.coarse_mode > 2 || !(o.coarse_rtol > 0.0)) return MG_EINVAL;
     if (o.coarse_restart < 1 || o.coarse_maxit < 1 || o.coarse_fixed_sweeps < 0) return MG_EINVAL;
-    if (o.restart < 1 || o.maxit < 1 || o.block_layout != 0) return MG_EINVAL;
+    if (o.restart < 1 || o.maxit < 1) return MG_EINVAL;
     if (o.kernel_variant < 0 || o.kernel_variant > 1) return MG_EINVAL;
     if (o.smoother < 0 || o.smoother > 1) return MG_EINVAL;
     if (!(o.orth_eta >= 0.0) || o.orth_eta >= 1.0) return MG_EINVAL;
@@ -1656,7 +1655,6 @@ int mg_update_options(mg_handle *h, const mg_options *opt) {
     o.free = h->opt.free;
     o.alloc_ctx = h->opt.alloc_ctx;
     o.eig_iters = h->opt.eig_iters;
-    o.block_layout = h->opt.block_layout;
     if (validate_options(o) != MG_OK) return MG_EINVAL;
     const bool bounds = (o.cheb_lo != h->opt.cheb_lo) || (o.cheb_hi != h->opt.cheb_hi);
     if ((o.kernel_variant != h->opt.kernel_variant || o.orth_eta != h->opt.orth_eta) && h->coarse_graph) {  // the captured cycle holds the old kernels

@@ -21,7 +21,8 @@ from gpu_util import gpu_solver, to_dev, to_np
 pytestmark = [pytest.mark.gpu, pytest.mark.slow]
 
 GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
-CASES = ["C0_direct", "C0_default", "C2r_direct", "C2r_default", "C3r_direct", "C3r_default", "C1_direct", "C2-16_direct"]
+CASES = ["C0_direct", "C0_default", "C2r_direct", "C2r_default", "C3r_direct", "C3r_default", "C1_direct", "C2-16_direct",
+         "C1_default_2its"]
 
 
 def load(case):
@@ -53,7 +54,8 @@ def test_solve_matches_oracle_golden(case):
         k = min(len(g["hist"]), len(info["hist"]))
         band = np.abs(np.log10(np.array(info["hist"][:k]) / np.array(g["hist"][:k])))
         assert band.max() <= 0.05, band.max()
-        assert info["rel_res"] <= 1.05 * g["rtol"]
+        if g["converged"]:
+            assert info["rel_res"] <= 1.05 * g["rtol"]
         if o["coarse_mode"] == 2:
             assert info["coarse_iters_total"] == 0
         print(f"{case}: iters {info['iters']} (oracle {g['iters']}), history band {band.max():.2e} decades, "

@@ -60,14 +60,16 @@ def test_vcycle_default_mode_residual_sense(case):
 
 
 @pytest.mark.parametrize("case", ["b12-3lev", "b6-4lev", "b5-generic-to-1-plane", "b36-3lev"])
-@pytest.mark.parametrize("graphs", [1, 0])
-def test_coarse_solve(case, graphs):
+@pytest.mark.parametrize("graphs,eta", [(1, 0.25), (0, 0.25), (1, 0.0)])
+def test_coarse_solve(case, graphs, eta):
     """PBJ-GMRES(100) to 1e-10 on the coarsest level: both reach the tolerance; the solutions agree to
-    cond * rtol.  The inner iteration COUNT is not a parity quantity (north_star's +-1 is for the outer FGMRES):
-    a restarted GMRES that needs ~60 restart cycles near stagnation amplifies the rounding difference between
-    CGS2 (device) and MGS (oracle) -- cf. PAPER.md:170, CPU and GPU counts of the same solver differ -- so the
-    count is only checked to a 15 % band (measured: 3296 vs 3076 on b12-3lev)."""
-    w, H, s = make(case, use_graphs=graphs)
+    cond * rtol.  The inner iteration COUNT is not a north_star parity quantity (its +-1 is for the outer FGMRES) and a
+    restarted GMRES near stagnation amplifies rounding differences between Gram-Schmidt variants (CPU and
+    GPU counts of the same solver differ), so it is held to a 5 % band -- measured in round 2 with classical Gram-Schmidt
+    + reorthogonalisation on every step (orth_eta = 0) and with selective reorthogonalisation (0.25) alike: 2959 / 2960 vs
+    2958 (oracle, MGS), 1944 vs 1944, 69 vs 69, 3865 / 3881 vs 3894.  (Round 1 had widened the band to 15 % after a
+    3296 vs 3076 mismatch of an earlier kernel; the 5 % band is restored.)"""
+    w, H, s = make(case, use_graphs=graphs, orth_eta=eta)
     try:
         Lc = H.levels[-1]
         r = input_vector(Lc.n, w.seed, 23)
@@ -79,12 +81,13 @@ def test_coarse_solve(case, graphs):
         assert np.linalg.norm(r - mg.spmv(Lc, e)) <= 1.01e-10 * rn       # the device solve met its tolerance
         assert np.linalg.norm(r - mg.spmv(Lc, e_or)) <= 1.01e-10 * rn
         assert np.linalg.norm(mg.spmv(Lc, e - e_or)) <= 2.1e-10 * rn
-        assert abs(it - it_or) <= max(2, int(0.15 * it_or))
+        print(f"coarse iterations: device {it} (orth_eta {eta}), oracle {it_or}")
+        assert abs(it - it_or) <= max(2, int(0.05 * it_or))
     finally:
         s.destroy()
 
 
-@pytest.mark.parametrize("case", ["b12-3lev", "b6-4lev", "b5-generic-to-1-plane"])
+@pytest.mark.parametrize("case", ["b12-3lev", "b6-4lev", "b5-generic-to-1-plane", "b36-3lev"])
 def test_solve_iteration_count_and_history(case):
     w, H, s = make(case)
     try:

@@ -47,6 +47,25 @@ def test_power_iteration_start_vector_and_estimate():
         assert L.lam_max == pytest.approx(1.1 * L.rho_est) and L.lam_min == pytest.approx(0.1 * L.rho_est)
 
 
+@pytest.mark.parametrize("iters", [1, 2, 20])
+def test_power_iteration_closed_form_on_a_circulant(iters):
+    """b = 1 periodic tridiagonal: M = D^-1 A = circ(a/d, 1, a/d) is symmetric with Fourier eigenvectors and eigenvalues
+    lambda_k = 1 + (2a/d) cos(2 pi k/n).  With c_k the Fourier coefficients of the hashed start vector, m power steps give
+    exactly rho_est = ||M^m v0|| / ||M^(m-1) v0|| = sqrt(sum |c_k|^2 lambda_k^(2m) / sum |c_k|^2 lambda_k^(2m-2)) -- a pin that an
+    off-by-one in the step count or a Rayleigh-quotient estimate (sum |c|^2 lambda^(2m-1) / sum |c|^2 lambda^(2m-2)) fails."""
+    n, d, a = 16, 2.5, -1.0
+    L = bsr_from_dense(circ(n, a, d, a), 1, 1, n)
+    L.dinv = mg.pbj_invert(L)
+    lam = 1.0 + (2.0 * a / d) * np.cos(2.0 * np.pi * np.arange(n) / n)
+    c2 = np.abs(np.fft.fft(mg.hashed_start_vector(n))) ** 2
+    m = iters
+    exact = np.sqrt(np.sum(c2 * lam ** (2 * m)) / np.sum(c2 * lam ** (2 * m - 2)))
+    assert mg.power_rho(L, iters) == pytest.approx(exact, rel=1e-12)
+    rayleigh = np.sum(c2 * lam ** (2 * m - 1)) / np.sum(c2 * lam ** (2 * m - 2))
+    off_by_one = np.sqrt(np.sum(c2 * lam ** (2 * m + 2)) / np.sum(c2 * lam ** (2 * m)))
+    assert abs(rayleigh - exact) > 1e-6 * exact and abs(off_by_one - exact) > 1e-9 * exact   # the pin separates them
+
+
 @pytest.mark.parametrize("nu", [1, 2, 3, 4])
 def test_chebyshev_error_polynomial_closed_form_scalar_modes(nu):
     """b = 1 periodic tridiagonal: D^-1 A has Fourier eigenvectors with lambda_k = 1 + (2a/d) cos(2 pi k/n);

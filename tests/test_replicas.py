@@ -63,7 +63,7 @@ def test_reference_arm_runs_on_rank_0_only():
     code = """
         import sys
         sys.argv = ["bench.py", "--impl", "reference", "--gpus", "2", "--steps", "1", "--warmup", "0", "--workload", "C0",
-                    "--cpu-seconds", "0.2"]
+                    "--ref-coarse-its", "5"]
         import bench
         sys.exit(bench.main())
     """
@@ -75,4 +75,5 @@ def test_reference_arm_runs_on_rank_0_only():
     import json
     line = json.loads(out0.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["cpu_baseline"]["kind"] == "oracle"
+    assert line["cpu_baseline"]["measured"]["coarse_gmres_iterations_timed"] == 5 and line["gpu_launches"] == 0
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["unit"] == "s"
