@@ -16,7 +16,8 @@ Pins (tests/test_oracle_*.py, ``-m "not gpu"``): dense mat-vec and SciPy BSR; LA
 error polynomial closed form, nu=1 = damped block Jacobi, carried residual; ``P 1 = 1``, ``P^T P`` closed
 forms, adjointness; dense ``P^T A P``, ``P^T L_N P = L_{N/2}/2``, Kronecker closed form at delta=0; V-cycle
 vs the dense two-grid operator, exactness on range(P), contraction; coarse solve and full solve vs dense
-LU; FGMRES with M=I vs SciPy GMRES, M=A^-1 in one iteration.  Iteration COUNTS on the synthetic configs
+LU; FGMRES with M=I vs SciPy GMRES, M=A^-1 in one iteration; line blocks (NEXT-4) vs the dense block-diagonal
+solve with the planes of a node gathered by index, Chebyshev error polynomial with D := the line blocks.  Iteration COUNTS on the synthetic configs
 are "parity unpinned" by the paper (it has no such workloads): only oracle <-> GPU agreement is checked.
 """
 from __future__ import annotations
@@ -85,6 +86,7 @@ class Level:
     lam_min: float = None
     lam_max: float = None
     pphi: np.ndarray = None  # interpolation from the next coarser level to this one, [n_phi, n_phi/2]
+    linv: np.ndarray = None  # NEXT-4: dense inverses of the toroidal-line blocks, [n_pol, n_phi*b, n_phi*b]
 
     @property
     def n_brows(self):
@@ -113,7 +115,8 @@ class Options:
     coarse_fixed_sweeps: int = 8
     restart: int = 100
     maxit: int = 400
-    smoother: int = 0  # 0: PBJ-Chebyshev (north_star); 1: nu iterations of PBJ-preconditioned GMRES
+    smoother: int = 0  # 0: PBJ-Chebyshev (north_star); 1: nu iterations of PBJ-preconditioned GMRES;
+    #                    2: Chebyshev preconditioned by toroidal-LINE block Jacobi (NEXT-4)
 
 
 @dataclass
@@ -156,6 +159,36 @@ def pbj_apply(L: Level, r: np.ndarray) -> np.ndarray:
     z = np.empty(L.n)
     _c().orc_pbj_apply(L.n_brows, L.b, _p(L.dinv), _p(r), _p(z))
     return z
+
+
+# ------------------------------------------------------------------------------------------------------------
+# NEXT-4  larger Jacobi blocks: "expanding the options for, and size of, the blocks in the PBJ smoothers
+# ... line subdomains (e.g., in the toroidal direction)".  The block of poloidal node i is the
+# (n_phi b) x (n_phi b) diagonal block of A that couples ALL planes of node i (a periodic block-tridiagonal matrix for the
+# stencils of this path); its inverse is written out densely here (LAPACK), the definition of block Jacobi.
+# ------------------------------------------------------------------------------------------------------------
+def line_invert(L: Level) -> np.ndarray:
+    N, n_pol, b = L.n_phi, L.n_pol, L.b
+    M = np.zeros((n_pol, N * b, N * b))
+    rows = np.repeat(np.arange(L.n_brows, dtype=np.int64), np.diff(L.row_ptr))
+    cols = L.col_idx.astype(np.int64)
+    for p in np.nonzero(rows % n_pol == cols % n_pol)[0]:
+        i, k, m = rows[p] % n_pol, rows[p] // n_pol, cols[p] // n_pol
+        M[i, k * b:(k + 1) * b, m * b:(m + 1) * b] += L.vals[p]
+    return np.linalg.inv(M)
+
+
+def line_apply(L: Level, r: np.ndarray) -> np.ndarray:
+    """z = blockdiag(line blocks)^-1 r: gather the planes of every node, dense mat-vec, scatter back."""
+    N, n_pol, b = L.n_phi, L.n_pol, L.b
+    rl = r.reshape(N, n_pol, b).transpose(1, 0, 2).reshape(n_pol, N * b)
+    zl = np.einsum("ipq,iq->ip", L.linv, rl)
+    return np.ascontiguousarray(zl.reshape(n_pol, N, b).transpose(1, 0, 2)).ravel()
+
+
+def prec_apply(L: Level, r: np.ndarray) -> np.ndarray:
+    """The Jacobi preconditioner of the level smoother: point blocks (PBJ) or, if set up, toroidal lines."""
+    return line_apply(L, r) if L.linv is not None else pbj_apply(L, r)
 
 
 # ------------------------------------------------------------------------------------------------------------
@@ -230,7 +263,7 @@ def power_rho(L: Level, iters: int = 20) -> float:
     v = v / np.linalg.norm(v)
     rho = 0.0
     for _ in range(iters):
-        w = pbj_apply(L, spmv(L, v))
+        w = prec_apply(L, spmv(L, v))
         rho = float(np.linalg.norm(w))
         v = w / rho
     return rho
@@ -245,13 +278,13 @@ def chebyshev(L: Level, rhs: np.ndarray, x0, nu: int, return_residual: bool = Fa
     delta = 0.5 * (L.lam_max - L.lam_min)
     sigma1 = theta / delta
     r = rhs.copy() if x0 is None else rhs - spmv(L, x)
-    z = pbj_apply(L, r)
+    z = prec_apply(L, r)
     rho = 1.0 / sigma1
     d = z / theta
     for k in range(nu):
         x = x + d
         r = r - spmv(L, d)
-        z = pbj_apply(L, r)
+        z = prec_apply(L, r)
         rho_new = 1.0 / (2.0 * sigma1 - rho)
         d = (rho_new * rho) * d + (2.0 * rho_new / delta) * z
         rho = rho_new
@@ -399,6 +432,8 @@ def setup(row_ptr, col_idx, vals, b: int, n_pol: int, n_phi: int, levels: int, o
     lv = []
     for l in range(levels):
         L.dinv = pbj_invert(L)
+        if opt.smoother == 2 and l < levels - 1:   # the coarsest level is solved, not smoothed: PBJ for its GMRES
+            L.linv = line_invert(L)
         L.rho_est = power_rho(L, opt.eig_iters)
         L.lam_min, L.lam_max = opt.cheb_lo * L.rho_est, opt.cheb_hi * L.rho_est
         lv.append(L)
