@@ -229,8 +229,9 @@ def static_config(w, opt: dict, smoother: str = "chebyshev", world: int = 1) -> 
     """The part of ``config`` that names the workload and the method: identical in the CUDA and the reference arm."""
     return {"workload": w.name, "n_pol": w.n_pol, "n_phi": w.n_phi, "b": w.b, "levels": w.levels, "unknowns": w.n, "nnzb": w.nnzb,
             "rtol": RTOL,
-            "cycle": f"V({opt['nu_pre']},{opt['nu_post']}) " + ("PBJ-GMRES smoother (the paper's, PAPER.md:95)" if smoother == "gmres"
-                                                                  else "PBJ-Chebyshev"),
+            "cycle": f"V({opt['nu_pre']},{opt['nu_post']}) " + {"gmres": "PBJ-GMRES smoother (the paper's, PAPER.md:95)",
+                                                                "line": "toroidal-line block-Jacobi Chebyshev (NEXT-4, PAPER.md:212-214)"
+                                                                }.get(smoother, "PBJ-Chebyshev"),
             "coarsest": ("direct (block-tridiagonal Schur inverses)" if opt["coarse_mode"] == 2 else
                          f"PBJ-GMRES({opt['coarse_restart']}) to {opt['coarse_rtol']:g}"),
             "fgmres_restart": opt["restart"], "parallelism": "replicas only" if world > 1 else "1 GPU",
@@ -329,6 +330,8 @@ def cuda_arm(args):
     extra = {}
     if args.smoother == "gmres":
         extra["smoother"] = 1
+    if args.smoother == "line":
+        extra["smoother"] = 2
     if args.nu > 0:
         extra.update(nu_pre=args.nu, nu_post=args.nu)
     if args.coarse_mode >= 0:
@@ -397,6 +400,8 @@ def cuda_arm(args):
     if rank == 0:
         dinfo = s.direct_info() if opt["coarse_mode"] == 2 else None
         direct_bytes = dinfo["bytes_per_solve"] if dinfo else 0
+        # (launch-chain fallback of the direct solve: hundreds of launches per solve are booked under "direct", no per-launch size)
+        direct_launch_bytes = direct_bytes if dinfo and dinfo["persistent"] else 0
         s.update_options(maxit=min(opt["maxit"], 2))
         s.profile_reset()
         s.profile_enable(True)
@@ -411,7 +416,7 @@ def cuda_arm(args):
                 continue
             mean_ms = t["ms"] / t["timed"]
             per_step_launches = c["launches"] / args.steps
-            nbytes = class_bytes(sizes, level, kind, restart_by_level, direct_bytes)
+            nbytes = class_bytes(sizes, level, kind, restart_by_level, direct_launch_bytes)
             share_ms = per_step_launches * mean_ms
             detail.append({"level": level, "kind": kind, "launches_per_step": per_step_launches, "mean_us": 1e3 * mean_ms,
                            "bytes_per_launch": nbytes, "GBps": (nbytes / mean_ms / 1e6) if nbytes else None,
@@ -449,7 +454,7 @@ def cuda_arm(args):
         solve_bytes = solve_bytes_from_counts(sizes, info["iters"], info["coarse_iters_total"], opt, direct_bytes=direct_bytes)
         solve_bytes_dram = solve_bytes_from_counts(sizes, info["iters"], info["coarse_iters_total"], opt, dram_true=True,
                                                    direct_bytes=direct_bytes)
-        vcycle_roof = None if args.smoother == "gmres" else {   # the byte model below is the Chebyshev cycle's
+        vcycle_roof = None if args.smoother != "chebyshev" else {   # the byte model below is the PBJ-Chebyshev cycle's
             "pinned_coarse_mode": {"ms": vc_ms, "bytes": vc_bytes, "GBps": vc_bytes / vc_ms / 1e6,
                                    "frac_of_measured_peak": vc_bytes / vc_ms / 1e6 / peak, "frac_of_8TBs_nominal": vc_bytes / vc_ms / 1e6 / 8000.0},
             "complete_outer_iteration": {"ms": 1e3 * t_dev / max(1, info["iters"]), "bytes": solve_bytes / max(1, info["iters"]),
@@ -563,8 +568,9 @@ def main():
     ap.add_argument("--max-outer", type=int, default=0,
                     help="profiling aid (ncu launch lists): cap the outer FGMRES iterations of every solve; the line is then "
                          "marked \"truncated\": true and is NOT a bench value")
-    ap.add_argument("--smoother", choices=["chebyshev", "gmres"], default="chebyshev",
-                    help="level smoother: PBJ-Chebyshev (default, the metric's configuration) or the paper's PBJ-GMRES (NEXT-1)")
+    ap.add_argument("--smoother", choices=["chebyshev", "gmres", "line"], default="chebyshev",
+                    help="level smoother: PBJ-Chebyshev (default, the metric's configuration), the paper's PBJ-GMRES (NEXT-1) or "
+                         "toroidal-line block-Jacobi Chebyshev (NEXT-4)")
     ap.add_argument("--levels", type=int, default=0,
                     help="override the number of MG levels of the workload (e.g. 5 on C1: coarsen to 1 plane as the paper does, "
                          "PAPER.md:181); not the metric's configuration")

@@ -80,7 +80,12 @@ typedef struct mg_options {
                                 128-bit-load kernel for every b (kept for A/B measurement) */
     int smoother;            /* 0 (default): PBJ-Chebyshev (BASELINE.json north_star); 1: nu iterations of right-PBJ-
                                 preconditioned GMRES without a convergence test -- the paper's own level smoother,
-                                "one iteration of GMRES preconditioned with PBJ", V(1,1) / V(6,6) */
+                                "one iteration of GMRES preconditioned with PBJ", V(1,1) / V(6,6);
+                                2: Chebyshev preconditioned by toroidal-LINE block Jacobi (the paper's
+                                outlook): the block of a poloidal node couples all its planes, a periodic
+                                block-tridiagonal system factorised at setup / refresh into explicit b x b inverses.  Needs
+                                b <= 48 and same-node couplings on planes k-1, k, k+1 only (MG_EINVAL otherwise); 2N-1 extra
+                                blocks per node and level.  The coarsest-level GMRES keeps PBJ. */
     double orth_eta;         /* Gram-Schmidt in (F)GMRES: 0 = classical Gram-Schmidt with a second pass on every step
                                 (CGS2); eta in (0,1) = the second pass only when ||w - V V^T w|| < eta ||w|| (selective
                                 reorthogonalisation, Daniel-Gragg-Kaufman-Stewart).  Same Arnoldi relation either way.
@@ -198,7 +203,8 @@ int mg_set_cheb_bounds(mg_handle *h, int level, double lam_min, double lam_max);
 #define MG_KIND_OTHER 8
 #define MG_KIND_CYCLE 9     /* one whole coarsest-level GMRES restart cycle in a single persistent kernel */
 #define MG_KIND_DIRECT 10   /* direct coarsest-level solve: the persistent cooperative kernel (or its launch-chain fallback) */
-#define MG_KIND_COUNT 11
+#define MG_KIND_LINE 11     /* toroidal-line block solve + Chebyshev direction update (smoother = 2) */
+#define MG_KIND_COUNT 12
 #define MG_PROFILE_MAX_LEVELS 32
 /* Launches are always counted per (level, kind).  on != 0 additionally brackets every kernel launch with a
  * CUDA event pair on the stream and books its duration; CUDA-graph replay is bypassed while that is on. */

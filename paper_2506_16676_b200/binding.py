@@ -13,7 +13,7 @@ import os
 from . import buildlib
 
 MG_OK, MG_EINVAL, MG_ENOMEM, MG_ESINGULAR, MG_ECUDA = 0, -1, -2, -3, -4
-KIND_NAMES = ("spmv", "resid", "sweep", "sweep_nod", "pbj", "restrict", "prolong", "orth", "other", "cycle", "direct")
+KIND_NAMES = ("spmv", "resid", "sweep", "sweep_nod", "pbj", "restrict", "prolong", "orth", "other", "cycle", "direct", "line")
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
 FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)

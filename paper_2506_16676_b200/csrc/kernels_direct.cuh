@@ -690,6 +690,7 @@ __global__ void __launch_bounds__(DS_THREADS, 1) direct_solve_persistent_kernel(
         // is still the sentinel has not been written yet and is loaded again
         {
             const int nr = (d.p[0].rb - d.p[0].ra) + (d.p[1].rb - d.p[1].ra);
+            int released = 0;   // packed stages of this step handed back so far
             for (int q0 = 0; q0 < nr; q0 += RPP) {
                 int pi, row;
                 const bool have = ds_row_of(d, q0 + tid / DS_TPR, pi, row);
@@ -752,42 +753,53 @@ __global__ void __launch_bounds__(DS_THREADS, 1) direct_solve_persistent_kernel(
 #pragma unroll
                 for (int o = DS_TPR / 2; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
                 if (have && sub == 0) ds_st(a.tb + P.toff + row, P.phase == 0 ? zv - acc : acc);
+                // the packed stages whose rows are all done (this pass and before) go back to the producer once every
+                // consumer warp is here: a very wide level set has more packed stages than the ring holds
+                asm volatile("bar.sync 1, %0;" ::"n"(DS_WARPS * 32) : "memory");
+                {
+                    const int qe = min(q0 + RPP, nr);   // rows [0, qe) of the CTA's share are done
+                    const int nr0 = d.p[0].rb - d.p[0].ra;
+                    const int d0 = qe >= nr0 ? d.p[0].nA : min(d.p[0].nA, qe / d.p[0].rps);   // (nA = 0 for a job without blocks)
+                    const int d1 = qe >= nr ? d.p[1].nA : (qe > nr0 ? min(d.p[1].nA, (qe - nr0) / d.p[1].rps) : 0);
+                    const int upto = d0 + d1;
+                    for (int i = released + tid; i < upto; i += DS_WARPS * 32) ds_mbar_arrive(&empty[(int)((cnt + i) % ST)]);
+                    released = upto;
+                }
             }
         }
-        // all rows of the step's packed stages are consumed once every consumer warp is here: hand the stages back
-        asm volatile("bar.sync 1, %0;" ::"n"(DS_WARPS * 32) : "memory");
-        for (int i = tid; i < d.nA; i += DS_WARPS * 32) ds_mbar_arrive(&empty[(int)((cnt + i) % ST)]);
         cnt += d.nA;
         DS_STAMP(1);
         // ---- (B) rows of S_k^-1 times t: the step's t (written by all CTAs) into shared memory, polled until complete
-        for (int i0 = 0; i0 < d.nt; i0 += 16 * DS_WARPS * 32) {   // 16 independent loads in flight per thread
-            double tv[16];
-#pragma unroll
-            for (int u = 0; u < 16; ++u) {
-                const int i = i0 + tid + u * DS_WARPS * 32;
-                tv[u] = i < d.nt ? ds_ld(a.tb + d.t0 + i) : 0.0;
-            }
-            bool again;
-            do {
-                again = false;
-#pragma unroll
-                for (int u = 0; u < 16; ++u)
-                    if (ds_missing(tv[u])) {
-                        tv[u] = ds_ld(a.tb + d.t0 + i0 + tid + u * DS_WARPS * 32);
-                        again = again || ds_missing(tv[u]);
-                    }
-            } while (again);
-#pragma unroll
-            for (int u = 0; u < 16; ++u) {
-                const int i = i0 + tid + u * DS_WARPS * 32;
-                if (i < d.nt) tsm[i] = tv[u];
-            }
-        }
-        asm volatile("bar.sync 1, %0;" ::"n"(DS_WARPS * 32) : "memory");
-        DS_STAMP(3);
+        const int nr0 = d.p[0].rb - d.p[0].ra, nr1 = d.p[1].rb - d.p[1].ra;
         {
-            const int nr0 = d.p[0].rb - d.p[0].ra, nr = nr0 + (d.p[1].rb - d.p[1].ra);
-            for (int i = warp; i < nr; i += DS_WARPS) {
+            constexpr int tbase = 0;
+            const int tlen = d.nt;
+            for (int i0 = 0; i0 < tlen; i0 += 16 * DS_WARPS * 32) {   // 16 independent loads in flight per thread
+                double tv[16];
+#pragma unroll
+                for (int u = 0; u < 16; ++u) {
+                    const int i = i0 + tid + u * DS_WARPS * 32;
+                    tv[u] = i < tlen ? ds_ld(a.tb + d.t0 + tbase + i) : 0.0;
+                }
+                bool again;
+                do {
+                    again = false;
+#pragma unroll
+                    for (int u = 0; u < 16; ++u)
+                        if (ds_missing(tv[u])) {
+                            tv[u] = ds_ld(a.tb + d.t0 + tbase + i0 + tid + u * DS_WARPS * 32);
+                            again = again || ds_missing(tv[u]);
+                        }
+                } while (again);
+#pragma unroll
+                for (int u = 0; u < 16; ++u) {
+                    const int i = i0 + tid + u * DS_WARPS * 32;
+                    if (i < tlen) tsm[i] = tv[u];
+                }
+            }
+            asm volatile("bar.sync 1, %0;" ::"n"(DS_WARPS * 32) : "memory");
+            DS_STAMP(3);
+            for (int i = warp; i < nr0 + nr1; i += DS_WARPS) {
                 const int pi = i < nr0 ? 0 : 1;
                 DsPiece P = d.p[0];
                 if (pi) P = d.p[1];
@@ -804,7 +816,7 @@ __global__ void __launch_bounds__(DS_THREADS, 1) direct_solve_persistent_kernel(
                     }
                     const int len2 = min(DS_SEG, P.n - sg * DS_SEG) >> 1;
                     const double2 *A2 = reinterpret_cast<const double2 *>(ring + (size_t)st * DS_SEG);
-                    const double2 *t2 = reinterpret_cast<const double2 *>(tsm + (P.toff - d.t0) + (size_t)sg * DS_SEG);
+                    const double2 *t2 = reinterpret_cast<const double2 *>(tsm + (P.toff - d.t0 - tbase) + (size_t)sg * DS_SEG);
                     int e = lane;
                     for (; e + 32 < len2; e += 64) {
                         const double2 v0 = A2[e], v1 = A2[e + 32];

@@ -154,6 +154,52 @@ __device__ __forceinline__ void gmres_update_dev(const GmresDev &s, const int j)
     else if (it >= s.maxit) { s.status[0] = 1; }
 }
 
+// The same update by ONE WARP with three scratch arrays of j + 2 doubles in shared memory: the column, the rotations and the
+// coefficients are fetched with coalesced independent loads and the rotation recurrence runs out of shared memory.  (The
+// one-thread version above walks ~4 j dependent global loads: ~13 us at j = 50, a third of the whole Gram-Schmidt kernel.)
+// Same arithmetic in the same order, so the results are bit-identical.
+__device__ __forceinline__ void gmres_update_warp(const GmresDev &s, const int j, const int lane, double *sc, double *scs, double *ssn) {
+    if (s.status[0] != 0) return;   // (uniform: every lane reads the same value)
+    for (int i = lane; i <= j; i += 32) {
+        sc[i] = __ldcg(s.h1 + i) + __ldcg(s.h2 + i);
+        if (i < j) {
+            scs[i] = __ldcg(s.cs + i);
+            ssn[i] = __ldcg(s.sn + i);
+        }
+    }
+    __syncwarp();
+    if (lane == 0) {
+        const double hn = sqrt(fmax(*s.nrm2, 0.0));
+        sc[j + 1] = hn;
+        *s.hnext = hn;
+        for (int i = 0; i < j; ++i) {
+            const double t = scs[i] * sc[i] + ssn[i] * sc[i + 1];
+            sc[i + 1] = -ssn[i] * sc[i] + scs[i] * sc[i + 1];
+            sc[i] = t;
+        }
+        const double denom = hypot(sc[j], sc[j + 1]);
+        const double csj = sc[j] / denom, snj = sc[j + 1] / denom;
+        s.cs[j] = csj;
+        s.sn[j] = snj;
+        sc[j] = denom;
+        sc[j + 1] = 0.0;
+        const double gj = s.g[j];
+        s.g[j + 1] = -snj * gj;
+        s.g[j] = csj * gj;
+        const int it = s.status[2] + 1;
+        s.status[2] = it;
+        s.status[1] = j + 1;
+        const double est = fabs(snj * gj);
+        s.hist[it] = est;
+        const bool breakdown = (hn == 0.0);
+        if (est <= *s.tol || breakdown) { s.status[0] = 1; s.status[3] = 1; }
+        else if (it >= s.maxit) { s.status[0] = 1; }
+    }
+    __syncwarp();
+    double *col = s.H + (size_t)j * (s.m + 1);
+    for (int i = lane; i <= j + 1; i += 32) col[i] = sc[i];
+}
+
 // w += sign * sum_{i<k} coef[i] V_i ; optionally nrm2 = <w, w> of the result (same deterministic scheme).
 // If kdev != nullptr the live count is min(k, *kdev).
 __global__ void __launch_bounds__(256) axpy_multi_kernel(const double *__restrict__ V, const int64_t stride, const int k,
@@ -252,7 +298,15 @@ struct OrthArgs {
     double eta2;           // selective reorthogonalisation (Daniel-Gragg-Kaufman-Stewart): the second pass is skipped
                            // when ||w - V h1||^2 >= eta2 ||w||^2, estimated as ||w||^2 - |h1|^2; 0 = always two passes
 };
-#ifndef MG_ORTH_STAMP   // development probe: per-phase clock stamps (compiled out in the library)
+#ifdef MG_ORTH_STAMPS   // development probe (compiled out in the library): per-phase global-timer stamps of CTA 0, by step j
+__device__ unsigned long long orth_stamps[16 * 256];
+#define MG_ORTH_STAMP(k) \
+    if (blockIdx.x == 0 && threadIdx.x == 0 && a.j < 256) { \
+        unsigned long long t__; \
+        asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t__)); \
+        orth_stamps[a.j * 16 + (k)] = t__; \
+    }
+#else
 #define MG_ORTH_STAMP(k)
 #endif
 constexpr int ORTH_THREADS = 512;
@@ -464,8 +518,9 @@ __global__ void __launch_bounds__(ORTH_THREADS, 1) gmres_orth_fused_kernel(const
         if (lane == 0) {
             *a.dev.nrm2 = t;
             *a.counter = 0;
-            gmres_update_dev(a.dev, a.j);
         }
+        __syncwarp();
+        gmres_update_warp(a.dev, a.j, lane, hd, hd + a.ld, hs);   // hd [2 ld] and hs [ld] are free by now (ld >= m + 2)
     }
     MG_ORTH_STAMP(10);
 }

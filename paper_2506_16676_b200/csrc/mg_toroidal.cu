@@ -15,6 +15,7 @@
 #include "kernels_bsr.cuh"
 #include "kernels_bsr_tma.cuh"
 #include "kernels_direct.cuh"
+#include "kernels_line.cuh"
 #include "kernels_setup.cuh"
 #include "kernels_vec.cuh"
 
@@ -38,6 +39,11 @@ struct Level {
     int64_t *part = nullptr;  // TMA kernel: first block row of each persistent CTA (tma_grid + 1 entries)
     int tma_grid = 0;
     double rho_est = 0.0, lam_min = 0.0, lam_max = 0.0;
+    // toroidal-line block Jacobi (opt.smoother = 2): block positions, explicit inverses G (N per node), W (N - 1 per node)
+    int64_t *lpos = nullptr;
+    double *lineG = nullptr, *lineW = nullptr;
+    bool line_ready = false;   // factorised for the current values
+    bool rho_is_line = false;  // rho_est was estimated with the line preconditioner
     double *x = nullptr, *r = nullptr, *d[2] = {nullptr, nullptr}, *pe = nullptr, *rhs = nullptr;
     std::vector<int64_t> h_row_ptr;  // host copies of the pattern (Galerkin symbolic phase)
     std::vector<int32_t> h_col_idx;
@@ -403,6 +409,67 @@ int sweep(mg_handle *h, const Level &L, const double *vin, const double *rin, do
     return launch_bsr(h, L, a);
 }
 
+// ------------------------------------------------------------------------------------------------ line blocks (NEXT-4)
+inline bool line_mode(const mg_handle *h, const Level &L) { return h->opt.smoother == 2 && L.line_ready; }
+
+// dout = c_d dold + c_z M_line^-1 rin ; if xacc: xacc += dout.   dout must differ from rin and dold.
+int line_apply(mg_handle *h, const Level &L, const double *rin, const double *dold, double *dout, double c_d, double c_z,
+               double *xacc = nullptr) {
+    if (L.n_brows == 0) return MG_OK;
+    KindScope scope(h, L.index, MG_KIND_LINE);
+    LineArgs a{};
+    a.vals = L.vals;
+    a.lpos = L.lpos;
+    a.G = L.lineG;
+    a.W = L.lineW;
+    a.rin = rin;
+    a.dold = dold;
+    a.dout = dout;
+    a.x = xacc;
+    a.c_d = c_d;
+    a.c_z = c_z;
+    a.n_pol = h->n_pol;
+    a.N = L.n_phi;
+    a.b = h->b;
+    a.done = nullptr;
+    LAUNCH(h, line_apply_kernel, (h->n_pol + LINE_WARPS - 1) / LINE_WARPS, LINE_WARPS * 32, 0, a);
+    CU(cudaGetLastError());
+    return MG_OK;
+}
+
+// Positions (once) and factorisation (setup and every refresh) of the line blocks of one level.
+int setup_level_line(mg_handle *h, Level &L) {
+    const int b = h->b, N = L.n_phi;
+    const size_t bb = (size_t)b * b;
+    L.line_ready = false;
+    if (L.n_brows == 0) return MG_OK;
+    if (L.lpos == nullptr) {
+        MG(dalloc_t(h, &L.lpos, 3 * (size_t)L.n_brows));
+        MG(dalloc_t(h, &L.lineG, (size_t)h->n_pol * N * bb));
+        MG(dalloc_t(h, &L.lineW, (size_t)h->n_pol * std::max(N - 1, 1) * bb));
+        int *bad = nullptr;
+        MG(dalloc_t(h, &bad, 4));
+        CU(cudaMemsetAsync(bad, 0, sizeof(int), h->stream));
+        LAUNCH(h, line_positions_kernel, grid_for(L.n_brows, 256, 1 << 30), 256, 0, L.row_ptr, L.col_idx, h->n_pol, N, L.lpos, bad);
+        int hbad = 0;
+        CU(cudaMemcpyAsync(&hbad, bad, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+        dfree_t(h, bad);
+        if (hbad) return MG_EINVAL;   // a node couples itself beyond the neighbouring planes: not a tridiagonal line block
+    }
+    const size_t smem = sizeof(double) * (7 * bb + b);
+    if (smem > 48 * 1024) CU(cudaFuncSetAttribute(line_factor_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CU(cudaMemsetAsync(L.err_flag, 0xff, sizeof(unsigned long long), h->stream));
+    LAUNCH(h, line_factor_kernel, (unsigned)h->n_pol, 128, smem, L.vals, L.lpos, h->n_pol, N, b, L.lineG, L.lineW, L.err_flag);
+    CU(cudaGetLastError());
+    unsigned long long herr = 0;
+    CU(cudaMemcpyAsync(&herr, L.err_flag, sizeof(herr), cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    if (herr != ~0ull) return MG_ESINGULAR;
+    L.line_ready = true;
+    return MG_OK;
+}
+
 // ------------------------------------------------------------------------------------------------ reductions
 // out[0] = <a, b> via the handle's scratch reduction (device result).
 int dot_dev(mg_handle *h, const double *a, const double *b, int64_t n, double *out) {
@@ -446,6 +513,17 @@ int presmooth(mg_handle *h, Level &L, const double *rhs, double *x, int nu) {
         return MG_OK;
     }
     const Cheb c = cheb_of(L);
+    if (line_mode(h, L)) {   // the same recurrence with D := the toroidal-line blocks; their solve is a kernel of its own
+        MG(line_apply(h, L, rhs, nullptr, L.d[0], 0.0, 1.0 / c.theta));
+        double rho = 1.0 / c.sigma1;
+        for (int k = 0; k < nu; ++k) {
+            const double rho_new = 1.0 / (2.0 * c.sigma1 - rho);
+            MG(sweep(h, L, L.d[k & 1], k == 0 ? rhs : L.r, L.r, x, nullptr, 0.0, 0.0, (k == 0) ? F_SET_X : F_UPD_X));
+            if (k < nu - 1) MG(line_apply(h, L, L.r, L.d[k & 1], L.d[(k + 1) & 1], rho_new * rho, 2.0 * rho_new / c.delta));
+            rho = rho_new;
+        }
+        return MG_OK;
+    }
     MG(pbj(h, L, rhs, L.d[0], 1.0 / c.theta));  // d_0 = D^-1 r_0 / theta, r_0 = rhs
     double rho = 1.0 / c.sigma1;
     for (int k = 0; k < nu; ++k) {
@@ -464,6 +542,18 @@ int presmooth(mg_handle *h, Level &L, const double *rhs, double *x, int nu) {
 int postsmooth(mg_handle *h, Level &L, const double *v, double *x, int nu) {
     if (nu <= 0) return MG_OK;
     const Cheb c = cheb_of(L);
+    if (line_mode(h, L)) {
+        MG(sweep(h, L, v, L.r, L.r, x, nullptr, 0.0, 0.0, 0));   // r -= A v
+        MG(line_apply(h, L, L.r, nullptr, L.d[0], 0.0, 1.0 / c.theta, nu == 1 ? x : nullptr));
+        double rho = 1.0 / c.sigma1;
+        for (int k = 0; k + 1 < nu; ++k) {
+            const double rho_new = 1.0 / (2.0 * c.sigma1 - rho);
+            MG(sweep(h, L, L.d[k & 1], L.r, L.r, x, nullptr, 0.0, 0.0, F_UPD_X));
+            MG(line_apply(h, L, L.r, L.d[k & 1], L.d[(k + 1) & 1], rho_new * rho, 2.0 * rho_new / c.delta, k == nu - 2 ? x : nullptr));
+            rho = rho_new;
+        }
+        return MG_OK;
+    }
     MG(sweep(h, L, v, L.r, L.r, x, L.d[0], 0.0, 1.0 / c.theta, F_NEED_D | (nu == 1 ? F_FINAL_X : 0)));
     double rho = 1.0 / c.sigma1;
     for (int k = 0; k + 1 < nu; ++k) {
@@ -954,22 +1044,20 @@ int direct_symbolic(mg_handle *h) {
             tcap = std::max(tcap, (nt + 1) / 2 * 2);
         }
         const size_t budget = 227 * 1024;
+        // (level sets so wide that the t of a step leaves fewer than DS_PL ring stages -- C3: 2 x 8,496 scalars -- take the
+        // launch chain: measured 10.06 ms against 10.32 ms per C3 coarse solve for a persistent variant with one job's t at a time)
         int stages = 0;
         if (direct_smem_bytes(DS_PL, tcap, nsteps) <= budget)
             stages = (int)std::min<size_t>(64, (budget - direct_smem_bytes(0, tcap, nsteps)) /
                                                    (sizeof(double) * DS_SEG + 2 * sizeof(uint64_t) + sizeof(int)));
         bool fits = (b % 2 == 0) && b >= DS_TPR && b <= 64 && ne_max <= DS_MAXNE && stages >= DS_PL && h->coop_launch;
-        for (size_t si = 0; fits && si < dc.steps.size(); ++si) {   // the packed stages of a step are handed back together
-            int nA = 0;
-            for (const auto &j : dc.steps[si]) {
-                const int rowlen = lev_ne[2 * j.level + j.phase] * b;
+        for (int k = 0; fits && k < dc.nlev; ++k)   // the packed stages of one pass of phase (A) are handed back together
+            for (int side = 0; side < 2; ++side) {
+                const int rowlen = lev_ne[2 * k + side] * b;
                 if (rowlen == 0) continue;
-                const int rps = DS_SEG / rowlen, nr = dc.nk[j.level] / h->sm_count + 2;
-                if (rps < 1) fits = false;
-                else nA += (nr + rps - 1) / rps;
+                const int rps = DS_SEG / rowlen, rpp = DS_WARPS * 32 / DS_TPR;
+                if (rps < 1 || (rpp + rps - 1) / rps + 2 > stages - 1) fits = false;
             }
-            if (nA > stages - 1) fits = false;
-        }
         int per_sm = 0;
         if (fits &&
             cudaFuncSetAttribute(direct_solve_persistent_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -1314,9 +1402,11 @@ int power_rho(mg_handle *h, Level &L, int iters, double *rho_out) {
     }
     LAUNCH(h, axpby_kernel, grid_for(L.nvec, 256), 256, 0, 1.0 / std::sqrt(nrm2), L.x, 0.0, L.x, L.nvec);
     double rho = 0.0;
+    L.rho_is_line = line_mode(h, L);
     for (int it = 0; it < iters; ++it) {
         MG(spmv(h, L, L.x, L.r));
-        MG(pbj(h, L, L.r, L.d[0], 1.0));
+        if (L.rho_is_line) MG(line_apply(h, L, L.r, nullptr, L.d[0], 0.0, 1.0));
+        else MG(pbj(h, L, L.r, L.d[0], 1.0));
         MG(dot_host(h, L.d[0], L.d[0], L.nvec, &nrm2));
         rho = std::sqrt(nrm2);
         if (!(rho > 0.0)) break;
@@ -1537,7 +1627,7 @@ static int validate_options(const mg_options &o) {
     if (o.coarse_restart < 1 || o.coarse_maxit < 1 || o.coarse_fixed_sweeps < 0) return MG_EINVAL;
     if (o.restart < 1 || o.maxit < 1) return MG_EINVAL;
     if (o.kernel_variant < 0 || o.kernel_variant > 1) return MG_EINVAL;
-    if (o.smoother < 0 || o.smoother > 1) return MG_EINVAL;
+    if (o.smoother < 0 || o.smoother > 2) return MG_EINVAL;
     if (!(o.orth_eta >= 0.0) || o.orth_eta >= 1.0) return MG_EINVAL;
     return MG_OK;
 }
@@ -1570,6 +1660,7 @@ int mg_setup(mg_handle **out, const int64_t *row_ptr, const int32_t *col_idx, co
     *out = nullptr;
     if (!row_ptr || !col_idx || !vals || !aligned16(vals)) return MG_EINVAL;
     if (b < 1 || b > 64 || n_pol < 1 || n_phi < 1 || levels < 1 || levels > 30) return MG_EINVAL;
+    if (opt && opt->smoother == 2 && b > 48) return MG_EINVAL;   // shared memory of the line factorisation
     if (n_phi % (1 << (levels - 1)) != 0) return MG_EINVAL;
     mg_options o;
     if (opt) o = *opt; else mg_options_default(&o);
@@ -1639,6 +1730,7 @@ int mg_setup(mg_handle **out, const int64_t *row_ptr, const int32_t *col_idx, co
         if ((rc = setup_level_pbj(h, L)) != MG_OK) return fail(rc);
         if ((rc = setup_level_partition(h, L)) != MG_OK) return fail(rc);
         if ((rc = alloc_level_vectors(h, L)) != MG_OK) return fail(rc);
+        if (o.smoother == 2 && l + 1 < levels && (rc = setup_level_line(h, L)) != MG_OK) return fail(rc);
         if ((rc = power_rho(h, L, o.eig_iters, &L.rho_est)) != MG_OK) return fail(rc);
         set_bounds(h, L);
         if (l + 1 < levels && (rc = build_coarse_level(h, l)) != MG_OK) return fail(rc);
@@ -1662,7 +1754,17 @@ int mg_update_options(mg_handle *h, const mg_options *opt) {
         cudaGraphExecDestroy(h->coarse_graph);
         h->coarse_graph = nullptr;
     }
+    if (o.smoother == 2 && h->b > 48) return MG_EINVAL;
     h->opt = o;
+    // the Chebyshev interval belongs to the preconditioner (point or line blocks): re-estimate where it changed
+    for (int l = 0; l + 1 < h->n_levels; ++l) {
+        Level &L = h->lev[l];
+        if (o.smoother == 2 && !L.line_ready) MG(setup_level_line(h, L));
+        if (L.rho_is_line != (o.smoother == 2)) {
+            MG(power_rho(h, L, o.eig_iters, &L.rho_est));
+            set_bounds(h, L);
+        }
+    }
     if (bounds)
         for (auto &L : h->lev) set_bounds(h, L);
     return MG_OK;
@@ -1681,6 +1783,8 @@ int mg_update_values(mg_handle *h, const double *vals) {
     for (int l = 0; l < h->n_levels; ++l) {
         Level &L = h->lev[l];
         MG(invert_level_blocks(h, L));
+        L.line_ready = false;
+        if (h->opt.smoother == 2 && l + 1 < h->n_levels) MG(setup_level_line(h, L));
         MG(power_rho(h, L, h->opt.eig_iters, &L.rho_est));
         set_bounds(h, L);
         if (l + 1 < h->n_levels) MG(galerkin_numeric(h, l));
@@ -1938,6 +2042,11 @@ const char *mg_strerror(int code) {
     }
 }
 
+#ifdef MG_ORTH_STAMPS
+int mg_debug_orth_stamps(unsigned long long *host, int n) {
+    return cudaMemcpyFromSymbol(host, mgk::orth_stamps, sizeof(unsigned long long) * n) == cudaSuccess ? 0 : -1;
+}
+#endif
 #ifdef MG_DS_STAMP
 int mg_debug_ds_stamps(unsigned long long *host, int n) {
     return cudaMemcpyFromSymbol(host, mgk::ds_stamps, sizeof(unsigned long long) * n) == cudaSuccess ? 0 : -1;
