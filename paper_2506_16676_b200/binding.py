@@ -117,12 +117,14 @@ def options_default(**kw) -> mg_options:
     return o
 
 
-def _ptr(t, dtype=None):
+def _ptr(t, dtype=None, numel=None):
     import torch
     if not isinstance(t, torch.Tensor) or not t.is_cuda or not t.is_contiguous():
         raise TypeError("expected a contiguous CUDA tensor")
     if dtype is not None and t.dtype != dtype:
         raise TypeError(f"expected dtype {dtype}, got {t.dtype}")
+    if numel is not None and t.numel() != numel:
+        raise ValueError(f"expected {numel} elements, got {t.numel()}")
     return C.c_void_p(t.data_ptr())
 
 
@@ -195,7 +197,7 @@ class Solver:
     def vcycle(self, r, z=None):
         import torch
         z = self.new() if z is None else z
-        _chk(lib().mg_vcycle(self._h, _ptr(r, torch.float64), _ptr(z, torch.float64)), "mg_vcycle")
+        _chk(lib().mg_vcycle(self._h, _ptr(r, torch.float64, self.n()), _ptr(z, torch.float64, self.n())), "mg_vcycle")
         return z
 
     def solve(self, rhs, x=None, rtol: float = 1e-8, x_is_initial_guess: bool = False, hist_cap: int = 0):
@@ -205,7 +207,7 @@ class Solver:
         hist = (C.c_double * hist_cap)() if hist_cap > 0 else None
         info.hist_len = hist_cap
         info.hist = C.cast(hist, C.POINTER(C.c_double)) if hist is not None else None
-        _chk(lib().mg_solve(self._h, _ptr(rhs, torch.float64), _ptr(x, torch.float64), float(rtol),
+        _chk(lib().mg_solve(self._h, _ptr(rhs, torch.float64, self.n()), _ptr(x, torch.float64, self.n()), float(rtol),
                             int(bool(x_is_initial_guess)), C.byref(info)), "mg_solve")
         return x, _info_dict(info, hist)
 
@@ -222,38 +224,38 @@ class Solver:
     def spmv(self, level, x, y=None):
         import torch
         y = self.new(level) if y is None else y
-        _chk(lib().mg_spmv(self._h, level, _ptr(x, torch.float64), _ptr(y, torch.float64)), "mg_spmv")
+        _chk(lib().mg_spmv(self._h, level, _ptr(x, torch.float64, self.n(level)), _ptr(y, torch.float64, self.n(level))), "mg_spmv")
         return y
 
     def residual(self, level, rhs, x, r=None):
         import torch
         r = self.new(level) if r is None else r
-        _chk(lib().mg_residual(self._h, level, _ptr(rhs, torch.float64), _ptr(x, torch.float64),
-                               _ptr(r, torch.float64)), "mg_residual")
+        _chk(lib().mg_residual(self._h, level, _ptr(rhs, torch.float64, self.n(level)), _ptr(x, torch.float64, self.n(level)),
+                               _ptr(r, torch.float64, self.n(level))), "mg_residual")
         return r
 
     def pbj_apply(self, level, r, z=None):
         import torch
         z = self.new(level) if z is None else z
-        _chk(lib().mg_pbj_apply(self._h, level, _ptr(r, torch.float64), _ptr(z, torch.float64)), "mg_pbj_apply")
+        _chk(lib().mg_pbj_apply(self._h, level, _ptr(r, torch.float64, self.n(level)), _ptr(z, torch.float64, self.n(level))), "mg_pbj_apply")
         return z
 
     def smooth(self, level, rhs, x, nu: int, zero_guess: bool):
         import torch
-        _chk(lib().mg_smooth(self._h, level, _ptr(rhs, torch.float64), _ptr(x, torch.float64), int(nu),
+        _chk(lib().mg_smooth(self._h, level, _ptr(rhs, torch.float64, self.n(level)), _ptr(x, torch.float64, self.n(level)), int(nu),
                              int(bool(zero_guess))), "mg_smooth")
         return x
 
     def restrict(self, level, r_fine, r_coarse=None):
         import torch
         r_coarse = self.new(level + 1) if r_coarse is None else r_coarse
-        _chk(lib().mg_restrict(self._h, level, _ptr(r_fine, torch.float64), _ptr(r_coarse, torch.float64)),
+        _chk(lib().mg_restrict(self._h, level, _ptr(r_fine, torch.float64, self.n(level)), _ptr(r_coarse, torch.float64, self.n(level + 1))),
              "mg_restrict")
         return r_coarse
 
     def prolong_add(self, level, e_coarse, x_fine):
         import torch
-        _chk(lib().mg_prolong_add(self._h, level, _ptr(e_coarse, torch.float64), _ptr(x_fine, torch.float64)),
+        _chk(lib().mg_prolong_add(self._h, level, _ptr(e_coarse, torch.float64, self.n(level + 1)), _ptr(x_fine, torch.float64, self.n(level))),
              "mg_prolong_add")
         return x_fine
 
@@ -261,7 +263,7 @@ class Solver:
         import torch
         e = self.new(self.levels - 1) if e is None else e
         it = C.c_int(0)
-        _chk(lib().mg_coarse_solve(self._h, _ptr(r, torch.float64), _ptr(e, torch.float64), C.byref(it)),
+        _chk(lib().mg_coarse_solve(self._h, _ptr(r, torch.float64, self.n(self.levels - 1)), _ptr(e, torch.float64, self.n(self.levels - 1)), C.byref(it)),
              "mg_coarse_solve")
         return e, it.value
 

@@ -81,3 +81,58 @@ def test_lagged_solve_matches_the_oracle():
         assert np.linalg.norm(w0.rhs - mg.spmv(L0, to_np(x0))) <= 1.05e-8 * np.linalg.norm(w0.rhs)
     finally:
         s.destroy()
+
+
+def test_refresh_with_one_level_rebuilds_the_captured_coarse_cycle():
+    """levels = 1: the coarsest level IS level 0, whose values pointer is borrowed; mg_update_values with a NEW buffer must not
+    leave the captured CUDA graph of the coarse GMRES cycle pointing at the old one."""
+    import torch
+    w = small("C0", mesh=(3, 8), n_phi=4, levels=1, b=6, seed=91)
+    H = oracle_hierarchy(w)
+    s = gpu_solver(w, inject_bounds_from=H)
+    try:
+        r = input_vector(w.n, 91, 24)
+        z1 = to_np(s.vcycle(to_dev(r)))                       # captures the graph on the first buffer
+        assert np.linalg.norm(r - mg.spmv(H.levels[0], z1)) <= 1.01e-10 * np.linalg.norm(r)
+        vals2 = (s.vals * 2.0).clone()                        # a new buffer with A' = 2 A
+        old = s.vals
+        s.update_values(vals2)
+        old.zero_()                                           # the old buffer must not be read any more
+        z2 = to_np(s.vcycle(to_dev(r)))
+        assert np.linalg.norm(r - 2.0 * mg.spmv(H.levels[0], z2)) <= 1.01e-10 * np.linalg.norm(r)
+    finally:
+        s.destroy()
+
+
+def test_changing_restart_and_maxit_does_not_leak_device_memory():
+    """Every change of restart / maxit used to allocate a new Krylov basis and keep the old one until mg_destroy."""
+    w = small("C0", mesh=(5, 16), n_phi=8, levels=3, b=12, seed=77)
+    s = gpu_solver(w, coarse_mode=1)
+    try:
+        rhs = to_dev(w.rhs)
+        s.update_options(restart=20, maxit=30)
+        s.solve(rhs, rtol=1e-8)
+        base = s.device_bytes()
+        for restart, maxit in ((10, 15), (20, 30), (20, 40), (35, 40), (20, 30)):
+            s.update_options(restart=restart, maxit=maxit)
+            s.solve(rhs, rtol=1e-8)
+        assert s.device_bytes() == base
+    finally:
+        s.destroy()
+
+
+def test_misaligned_and_wrong_size_vectors_are_rejected():
+    import torch
+    from paper_2506_16676_b200 import binding
+    w = small("C0", mesh=(3, 8), n_phi=4, levels=2, b=6, seed=92)
+    s = gpu_solver(w)
+    try:
+        buf = torch.zeros(w.n + 1, dtype=torch.float64, device="cuda")
+        good = torch.zeros(w.n, dtype=torch.float64, device="cuda")
+        with pytest.raises(binding.MgError) as e:
+            s.spmv(0, buf[1:], good)                          # 8-byte, not 16-byte aligned
+        assert e.value.code == binding.MG_EINVAL
+        with pytest.raises((binding.MgError, ValueError, TypeError)):
+            s.spmv(0, buf[: w.n - 2], good)                    # too short
+    finally:
+        s.destroy()
