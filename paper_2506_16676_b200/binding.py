@@ -166,12 +166,15 @@ class Solver:
         self.destroy()
 
     # ---- helpers -------------------------------------------------------------------------------------------
-    def n(self, level: int = 0) -> int:
+    def n(self, level: int = 0):
+        """Vector length of a level (None for a level that does not exist: the library rejects it with MG_EINVAL)."""
+        if not 0 <= level < self.levels:
+            return None
         return (self.n_phi >> level) * self.n_pol * self.b
 
     def new(self, level: int = 0):
         import torch
-        return torch.empty(self.n(level), dtype=torch.float64, device=self.device)
+        return torch.empty(self.n(level) or 0, dtype=torch.float64, device=self.device)
 
     def update_options(self, **kw):
         for k, v in kw.items():
