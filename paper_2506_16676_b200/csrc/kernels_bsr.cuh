@@ -58,23 +58,23 @@ struct BsrCfg {
     static constexpr int EPR = B / VEC;      // elements per row of a block
     static constexpr int G = (EPB >= 256) ? 1 : (256 / EPB);  // block rows (groups) per CTA
     static constexpr int THREADS = ((G * EPB + 31) / 32) * 32;
+    static constexpr int RESIDENT = 2048 / THREADS;   // CTAs per SM the small-block kernel is compiled for (32 registers;
+                                                      // 5 / 6 CTAs with 48 / 40 registers measured 8-20 % slower)
 };
 
 // Small blocks are occupancy bound (ncu: 44 registers allowed 5 CTAs of 224 threads per SM, 55 % occupancy, DRAM at
 // 48 %): capping the kernel at 32 registers (full occupancy, 17 words of spill) raised b = 12 from 0.54 to 0.72 and
 // b = 6 from 0.53 to 0.62 of 8 TB/s.
+// One group of G block rows (row group `rg`) by one CTA; every return below is CTA-uniform.
 template <int B>
-__global__ void __launch_bounds__(BsrCfg<B>::THREADS, (B <= 12 ? 2048 / BsrCfg<B>::THREADS : 0)) bsr_fused_kernel(const BsrArgs a) {
+__device__ __forceinline__ void bsr_fused_rowgroup(const BsrArgs &a, const int64_t rg, double (*part)[BsrCfg<B>::EPB],
+                                                   double (*vec)[B]) {
     using C = BsrCfg<B>;
     constexpr int VEC = C::VEC, EPB = C::EPB, EPR = C::EPR, G = C::G, BB = B * B;
-    if (a.done != nullptr && *a.done != 0) return;
-    __shared__ double part[G][EPB];
-    __shared__ double vec[G][B];
-
     const int tid = threadIdx.x;
     const int g = tid / EPB;
     const int q = tid - g * EPB;
-    const int64_t I = (int64_t)blockIdx.x * G + g;
+    const int64_t I = rg * G + g;
     const bool valid = (g < G) && (I < a.n_brows);
     const int c = (q * VEC) % B;  // first column this thread multiplies
 
@@ -185,6 +185,23 @@ __global__ void __launch_bounds__(BsrCfg<B>::THREADS, (B <= 12 ? 2048 / BsrCfg<B
         a.dout[gi] = dnew;
         if (a.flags & F_FINAL_X) xv += dnew;
         if (touch_x) a.x[gi] = xv;
+    }
+}
+
+// The kernel: a grid-stride loop over the row groups.  Small blocks are launched with a RESIDENT grid (SM count x CTAs per SM):
+// a CTA lives for ~3 dependent load rounds per row group, so one CTA per group spent ~5-7 % of the launch on CTA turnover
+// (round 2, C4: b = 6 SpMV 4.88-4.93 -> 5.16-5.21 TB/s, sweep 4.67 -> 4.98-5.02; b = 12 SpMV 5.73-5.82 -> 5.86-6.08, sweep
+// 5.22-5.27 -> 5.55-5.62).
+template <int B>
+__global__ void __launch_bounds__(BsrCfg<B>::THREADS, (B <= 12 ? BsrCfg<B>::RESIDENT : 0)) bsr_fused_kernel(const BsrArgs a) {
+    using C = BsrCfg<B>;
+    if (a.done != nullptr && *a.done != 0) return;
+    __shared__ double part[C::G][C::EPB];
+    __shared__ double vec[C::G][B];
+    const int64_t ngroups = (a.n_brows + C::G - 1) / C::G;
+    for (int64_t rg = blockIdx.x; rg < ngroups; rg += gridDim.x) {
+        bsr_fused_rowgroup<B>(a, rg, part, vec);
+        __syncthreads();   // part / vec are reused by the next row group
     }
 }
 

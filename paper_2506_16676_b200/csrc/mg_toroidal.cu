@@ -347,7 +347,8 @@ int launch_bsr(mg_handle *h, const Level &L, BsrArgs a, TmaExtra ex = TmaExtra{}
     switch (h->b) {
 #define BSR_CASE(B)                                                                                          \
     case B: {                                                                                                \
-        const int grid = (int)((L.n_brows + BsrCfg<B>::G - 1) / BsrCfg<B>::G);                                \
+        int grid = (int)((L.n_brows + BsrCfg<B>::G - 1) / BsrCfg<B>::G);                                      \
+        if (B <= 12) grid = std::min(grid, h->sm_count * BsrCfg<B>::RESIDENT); /* resident grid, row groups in a loop */ \
         LAUNCH(h, bsr_fused_kernel<B>, grid, BsrCfg<B>::THREADS, 0, a);                                       \
         break;                                                                                               \
     }
