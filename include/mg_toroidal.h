@@ -48,6 +48,7 @@ extern "C" {
 #define MG_ENOMEM (-2)    /* device or host allocation failed */
 #define MG_ESINGULAR (-3) /* a diagonal block is missing or has a zero pivot (PBJ inverse undefined) */
 #define MG_ECUDA (-4)     /* CUDA runtime error; mg_strerror gives the last CUDA message */
+#define MG_ETOOLARGE (-5) /* mg_dot_noalloc: n exceeds MG_NOALLOC_MAX_N, the capacity of the library's fixed scratch array */
 
 typedef struct mg_handle mg_handle; /* opaque */
 
@@ -191,6 +192,25 @@ int mg_copy_level_to_host(mg_handle *h, int level, int64_t *row_ptr_host, int32_
                           double *dinv_host);
 /* Override the Chebyshev interval of one level (parity tests inject the oracle's bounds). */
 int mg_set_cheb_bounds(mg_handle *h, int level, double lam_min, double lam_max);
+/* ---- dot products (the reduction of the orthogonalisation: deterministic, warp-shuffle + fixed-order sums) -- */
+/* out[0] = <a, b> over the n_brows(level)*b entries of two level vectors; out is a DEVICE pointer (1 double), written on
+ * the handle's stream.  Scratch: the handle's own (allocated in mg_setup). */
+int mg_dot(mg_handle *h, int level, const double *a, const double *b, double *out);
+
+/* mg_dot_noalloc -- the same reduction (same kernel, same launch shape, hence the same bits as mg_dot) for callers that
+ * must not allocate: code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  It needs NO
+ * handle and calls no cudaMalloc / cudaFree / allocating routine: the per-CTA partial sums and the ticket counter live in a
+ * file-scope `static __device__` array of the library (MG_NOALLOC_SCRATCH_BYTES = 8,448 bytes; every GPU that loads the
+ * library holds it until exit), whose device address is taken once per device with cudaGetSymbolAddress.
+ *   a, b: DEVICE vectors of n doubles (16-byte aligned), out: DEVICE pointer to 1 double, cuda_stream: a cudaStream_t.
+ *   n <= MG_NOALLOC_MAX_N, else MG_ETOOLARGE (nothing is launched).  n == 0 gives 0.
+ * Every call shares the one scratch array: the ticket counter is cleared on the stream before each launch, the partial
+ * sums are overwritten before they are read.  Calls that OVERLAP on the GPU (different streams, or several host threads
+ * on one device) RACE on it: serialise them (one stream, or events).  Errors: MG_EINVAL, MG_ETOOLARGE, MG_ECUDA. */
+#define MG_NOALLOC_MAX_N ((int64_t)1 << 26)      /* 67,108,864 doubles = 512 MiB per vector (the configs' largest: 9,216,000) */
+#define MG_NOALLOC_SCRATCH_BYTES (1024 * 8 + 256)
+int mg_dot_noalloc(const double *a, const double *b, int64_t n, double *out, void *cuda_stream);
+
 /* ---- profiling: per-(level, kind) device time of the library's own kernel launches --------------------- */
 #define MG_KIND_SPMV 0      /* y = A x */
 #define MG_KIND_RESID 1     /* r = rhs - A x */

@@ -12,7 +12,8 @@ import os
 
 from . import buildlib
 
-MG_OK, MG_EINVAL, MG_ENOMEM, MG_ESINGULAR, MG_ECUDA = 0, -1, -2, -3, -4
+MG_OK, MG_EINVAL, MG_ENOMEM, MG_ESINGULAR, MG_ECUDA, MG_ETOOLARGE = 0, -1, -2, -3, -4, -5
+NOALLOC_MAX_N = 1 << 26
 KIND_NAMES = ("spmv", "resid", "sweep", "sweep_nod", "pbj", "restrict", "prolong", "orth", "other", "cycle", "direct", "line")
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
@@ -54,6 +55,8 @@ SYMBOLS = {
     "mg_prolong_add": (_I, [_VP, _I, _VP, _VP]),
     "mg_coarse_solve": (_I, [_VP, _VP, _VP, C.POINTER(_I)]),
     "mg_direct_info": (_I, [_VP, C.POINTER(_I), C.POINTER(_I64), C.POINTER(_I64), C.POINTER(_I), C.POINTER(_I)]),
+    "mg_dot": (_I, [_VP, _I, _VP, _VP, _VP]),
+    "mg_dot_noalloc": (_I, [_VP, _VP, _I64, _VP, _VP]),
     "mg_get_level": (_I, [_VP, _I, C.POINTER(_I64), C.POINTER(_I64), C.POINTER(_VP), C.POINTER(_VP), C.POINTER(_VP),
                           C.POINTER(_VP), C.POINTER(_D), C.POINTER(_D), C.POINTER(_D)]),
     "mg_copy_level_to_host": (_I, [_VP, _I, _VP, _VP, _VP, _VP]),
@@ -278,6 +281,14 @@ class Solver:
         return dict(level_sets=ls.value, dense_bytes=dense.value, offdiag_bytes=od.value, max_n=mx.value,
                     persistent=bool(pers.value), bytes_per_solve=2 * dense.value + od.value)
 
+    def dot(self, level, a, b, out=None):
+        """<a, b> of two level vectors into a 1-element device tensor (the handle's own scratch)."""
+        import torch
+        out = torch.empty(1, dtype=torch.float64, device=self.device) if out is None else out
+        _chk(lib().mg_dot(self._h, level, _ptr(a, torch.float64, self.n(level)), _ptr(b, torch.float64, self.n(level)),
+                          _ptr(out, torch.float64, 1)), "mg_dot")
+        return out
+
     def get_level(self, level: int) -> dict:
         """Sizes, Chebyshev bounds and (as torch views of the library's device memory) the level's arrays."""
         nb, nz = C.c_int64(), C.c_int64()
@@ -329,6 +340,18 @@ class Solver:
 
     def device_bytes(self) -> int:
         return int(lib().mg_device_bytes(self._h))
+
+
+def dot_noalloc(a, b, out):
+    """mg_dot_noalloc: <a, b> into the caller's 1-element device tensor ``out``; the library allocates nothing (its scratch is
+    a fixed device array; at most NOALLOC_MAX_N elements; calls that overlap on the GPU race on that array)."""
+    import torch
+    if a.numel() != b.numel():
+        raise ValueError("a and b differ in length")
+    stream = torch.cuda.current_stream().cuda_stream
+    _chk(lib().mg_dot_noalloc(_ptr(a, torch.float64), _ptr(b, torch.float64), a.numel(), _ptr(out, torch.float64, 1),
+                              C.c_void_p(stream)), "mg_dot_noalloc")
+    return out
 
 
 def _info_dict(info, hist):

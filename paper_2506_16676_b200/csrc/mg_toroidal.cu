@@ -8,6 +8,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <queue>
 #include <string>
 #include <vector>
@@ -24,6 +25,16 @@ using namespace mgk;
 namespace {
 
 thread_local std::string g_last_cuda_error;
+
+// ---- mg_dot_noalloc: scratch of the deterministic dot product in a file-scope device array (no cudaMalloc anywhere on that
+// path).  Layout: [0, 8192) 1,024 per-CTA partial sums (double), [8192, 8196) the ticket counter (unsigned).  In HOST code this
+// name is only a stand-in for the symbol: the device address comes from cudaGetSymbolAddress, once per device.
+constexpr int NOALLOC_MAX_GRID = 1024;
+static __device__ __align__(256) unsigned char mg_noalloc_scratch[MG_NOALLOC_SCRATCH_BYTES];
+static_assert(MG_NOALLOC_SCRATCH_BYTES >= NOALLOC_MAX_GRID * 8 + 4, "scratch holds the partial sums and the counter");
+constexpr int NOALLOC_MAX_DEVICES = 64;
+unsigned char *g_noalloc_ptr[NOALLOC_MAX_DEVICES] = {};   // device address of mg_noalloc_scratch per device ordinal
+std::mutex g_noalloc_mutex;
 
 struct Level {
     int index = 0;
@@ -2032,6 +2043,38 @@ int mg_profile_get(mg_handle *h, int level, int kind, int64_t *launches, int64_t
 int64_t mg_launch_count(mg_handle *h) { return h ? h->launches : -1; }
 int64_t mg_device_bytes(mg_handle *h) { return h ? h->dev_bytes : -1; }
 
+int mg_dot(mg_handle *h, int level, const double *a, const double *b, double *out) {
+    if (!level_ok(h, level) || !a || !b || !out || !aligned16(a) || !aligned16(b)) return MG_EINVAL;
+    return dot_dev(h, a, b, h->lev[level].nvec, out);
+}
+
+int mg_dot_noalloc(const double *a, const double *b, int64_t n, double *out, void *cuda_stream) {
+    if (!a || !b || !out || n < 0 || !aligned16(a) || !aligned16(b)) return MG_EINVAL;
+    if (n > MG_NOALLOC_MAX_N) return MG_ETOOLARGE;
+    int dev = -1;
+    CU(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return MG_EINVAL;
+    unsigned char *scratch = nullptr;
+    {   // once per device, with that device current: the device address of the file-scope array
+        std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+        if (g_noalloc_ptr[dev] == nullptr) {
+            void *p = nullptr;
+            CU(cudaGetSymbolAddress(&p, mg_noalloc_scratch));
+            g_noalloc_ptr[dev] = static_cast<unsigned char *>(p);
+        }
+        scratch = g_noalloc_ptr[dev];
+    }
+    cudaStream_t stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    double *partial = reinterpret_cast<double *>(scratch);
+    unsigned *counter = reinterpret_cast<unsigned *>(scratch + NOALLOC_MAX_GRID * sizeof(double));
+    // the array keeps the last call's contents: the ticket must start at zero (the partials are written before they are read)
+    CU(cudaMemsetAsync(counter, 0, sizeof(unsigned), stream));
+    const int grid = grid_for(n / 2 + 1, 256 * 4, NOALLOC_MAX_GRID);   // the launch shape of dot_dev: same sums, same order
+    dot_multi_kernel<<<dim3(grid, 1), 256, 0, stream>>>(a, (int64_t)0, b, n, partial, counter, out, (const int *)nullptr);
+    CU(cudaGetLastError());
+    return MG_OK;
+}
+
 const char *mg_strerror(int code) {
     switch (code) {
         case MG_OK: return "ok";
@@ -2039,6 +2082,7 @@ const char *mg_strerror(int code) {
         case MG_ENOMEM: return "out of memory";
         case MG_ESINGULAR: return "a diagonal block is missing or singular";
         case MG_ECUDA: return g_last_cuda_error.empty() ? "CUDA error" : g_last_cuda_error.c_str();
+        case MG_ETOOLARGE: return "mg_dot_noalloc: n exceeds MG_NOALLOC_MAX_N (2^26 doubles), the capacity of the fixed scratch array";
         default: return "unknown error code";
     }
 }
