@@ -377,4 +377,166 @@ __global__ void __launch_bounds__(LINE_WARPS * 32) line_apply_kernel(const LineA
     }
 }
 
+
+// ================================================================================================ staged apply (b % 4 == 0)
+// The same recurrences as line_apply_kernel, as a list of 5 (N - 1) mat-vec OPERATIONS per node executed by one CTA:
+// thread t owns the b/4-element segment t % 4 of row t / 4 of every block (the mapping of the b = 36 TMA kernel: the four
+// partial sums of a row meet by two shuffles).  The blocks an apply reads are STATIC, so thread 0 walks the operation list
+// ahead of the arithmetic with 1-D bulk async copies (TMA engine, SASS UBLKCP) into a ring of LS_STAGES block buffers: the
+// block of an operation is in shared memory before the operation starts, and every global read of a block is one coalesced
+// copy.  (line_apply_kernel walks the same ~5N dependent mat-vecs with per-lane row reads: 32 different lines per load
+// instruction, 2.5 TB/s on C1's level 0.)
+constexpr int LS_STAGES = 3;
+enum { LA_Q = 0, LA_Y, LA_T, LA_X, LA_B1, LA_B2, LA_ZN, LA_W };           // what the writer lanes do with the result t
+enum { LV_Y = 0, LV_Q, LV_X, LV_T, LV_Y2, LV_ZN, LV_COUNT };               // vectors in shared memory (64 doubles each)
+struct LineOp {
+    const double *M;   // b x b block (nullptr: absent, t = 0)
+    short src, act;    // source vector, action
+    int k;             // plane the action refers to
+};
+inline size_t line_staged_smem(int b, int N) {
+    const int nops = 5 * (N > 1 ? N - 1 : 0) + 1;
+    return sizeof(double) * ((size_t)LS_STAGES * b * b + LV_COUNT * 64) + sizeof(LineOp) * (size_t)nops + sizeof(uint64_t) * LS_STAGES + 64;
+}
+__device__ __forceinline__ uint32_t ls_smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void ls_issue(double *dst, const double *src, uint32_t bytes, uint64_t *bar) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(ls_smem_u32(bar)), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(ls_smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(ls_smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void ls_wait(uint64_t *bar, uint32_t parity) {
+    uint32_t ok;
+    do {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n"
+            : "=r"(ok)
+            : "r"(ls_smem_u32(bar)), "r"(parity)
+            : "memory");
+    } while (!ok);
+}
+
+// One CTA of 4 b threads per poloidal node.  Dynamic shared memory: line_staged_smem(b, N).
+__global__ void line_apply_staged_kernel(const LineArgs a) {
+    if (a.done != nullptr && *a.done != 0) return;
+    extern __shared__ __align__(128) unsigned char ls_raw[];
+    const int b = a.b, N = a.N, C = N - 1, bb = b * b, i = blockIdx.x, tid = threadIdx.x;
+    double *ring = reinterpret_cast<double *>(ls_raw);
+    double *vecs = ring + (size_t)LS_STAGES * bb;
+    LineOp *ops = reinterpret_cast<LineOp *>(vecs + LV_COUNT * 64);
+    const int nops = C > 0 ? 5 * C : 1;
+    uint64_t *full = reinterpret_cast<uint64_t *>(ops + nops);
+    const double *Gi = a.G + (size_t)i * N * bb;
+    const double *Wi = a.W + (size_t)i * (C > 0 ? C : 1) * bb;
+    auto blk = [&](int k, int which) -> const double * {
+        const int64_t p = a.lpos[3 * ((int64_t)k * a.n_pol + i) + which];
+        return p >= 0 ? a.vals + (size_t)p * bb : nullptr;
+    };
+    auto idx = [&](int k, int r) { return ((size_t)k * a.n_pol + i) * b + r; };
+    // ---- the operation list (closed form; see the top of the file)
+    for (int j = tid; j < nops; j += blockDim.x) {
+        LineOp o;
+        o.M = nullptr; o.src = LV_Y; o.act = LA_ZN; o.k = N - 1;
+        if (C == 0) {
+            o.M = Gi;                                                     // S^-1 = D_0^-1
+        } else if (j < 2 * C - 1) {                                       // forward: G_0 | L_k, G_k
+            const int k = (j + 1) / 2;
+            if ((j & 1) == 0) { o.M = Gi + (size_t)k * bb; o.src = LV_Y; o.act = LA_Q; o.k = k; }
+            else { o.M = blk(k, 0); o.src = LV_Q; o.act = LA_Y; o.k = k; }
+        } else if (j < 4 * C - 3) {                                       // backward: U_k, G_k for k = C-2 .. 0
+            const int m = j - (2 * C - 1), k = C - 2 - m / 2;
+            if ((m & 1) == 0) { o.M = blk(k, 2); o.src = LV_X; o.act = LA_T; o.k = k; }
+            else { o.M = Gi + (size_t)k * bb; o.src = LV_T; o.act = LA_X; o.k = k; }
+        } else if (j < 4 * C) {                                           // border
+            const int m = j - (4 * C - 3);
+            if (m == 0) { o.M = blk(N - 1, 2); o.src = LV_X; o.act = LA_B1; }
+            else if (m == 1) { o.M = blk(N - 1, 0); o.src = LV_Y2; o.act = LA_B2; }
+            else { o.M = Gi + (size_t)(N - 1) * bb; o.src = LV_Y; o.act = LA_ZN; }
+        } else {                                                          // z_k = x_k - W_k z_{N-1}
+            const int k = j - 4 * C;
+            o.M = Wi + (size_t)k * bb; o.src = LV_ZN; o.act = LA_W; o.k = k;
+        }
+        ops[j] = o;
+    }
+    if (tid == 0) {
+        for (int s = 0; s < LS_STAGES; ++s)
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(ls_smem_u32(&full[s])) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    const int r = tid >> 2, h = tid & 3, seg = b >> 2;
+    const bool active = r < b, writer = active && h == 0;
+    if (writer) vecs[LV_Y * 64 + r] = a.rin[idx(0, r)];                   // y_0 = r_0 (N = 1: the only right-hand side)
+    __syncthreads();
+    // ---- thread 0 keeps LS_STAGES block copies in flight, in list order (absent blocks take no stage)
+    int issue = 0, issued = 0;                                            // next list entry to look at / copies issued (thread 0)
+    auto issue_next = [&]() {
+        while (issue < nops && ops[issue].M == nullptr) ++issue;
+        if (issue < nops) {
+            ls_issue(ring + (size_t)(issued % LS_STAGES) * bb, ops[issue].M, (uint32_t)(bb * sizeof(double)), &full[issued % LS_STAGES]);
+            ++issue;
+            ++issued;
+        }
+    };
+    if (tid == 0)
+        for (int s = 0; s < LS_STAGES; ++s) issue_next();
+    double *z = a.dout;
+    int seq = 0;                                                          // copies consumed so far (every thread)
+    for (int j = 0; j < nops; ++j) {
+        const LineOp o = ops[j];
+        // values the action needs from global memory: asked for before the block is waited for
+        double g0 = 0.0;
+        if (writer) {
+            if (o.act == LA_Y) g0 = a.rin[idx(o.k, r)];
+            else if (o.act == LA_X || o.act == LA_W) g0 = z[idx(o.k, r)];
+            else if (o.act == LA_B2) g0 = a.rin[idx(N - 1, r)];
+            else if (o.act == LA_B1 && C > 1) g0 = z[idx(C - 1, r)];
+        }
+        double t = 0.0;
+        if (o.M != nullptr) {
+            ls_wait(&full[seq % LS_STAGES], (uint32_t)(seq / LS_STAGES) & 1u);
+            if (active) {
+                const double *Mrow = ring + (size_t)(seq % LS_STAGES) * bb + (size_t)r * b + h * seg;
+                const double *v = vecs + o.src * 64 + h * seg;
+                double t0 = 0.0, t1 = 0.0;
+                int cidx = 0;
+                for (; cidx + 1 < seg; cidx += 2) {
+                    t0 = fma(Mrow[cidx], v[cidx], t0);
+                    t1 = fma(Mrow[cidx + 1], v[cidx + 1], t1);
+                }
+                if (cidx < seg) t0 = fma(Mrow[cidx], v[cidx], t0);
+                t = t0 + t1;
+            }
+            t += __shfl_xor_sync(0xffffffffu, t, 1);
+            t += __shfl_xor_sync(0xffffffffu, t, 2);
+            ++seq;
+        }
+        if (writer) {
+            double *V = vecs;
+            switch (o.act) {
+                case LA_Q: V[LV_Q * 64 + r] = t; V[LV_X * 64 + r] = t; z[idx(o.k, r)] = t; break;
+                case LA_Y: V[LV_Y * 64 + r] = g0 - t; break;
+                case LA_T: V[LV_T * 64 + r] = t; break;
+                case LA_X: { const double xv = g0 - t; V[LV_X * 64 + r] = xv; z[idx(o.k, r)] = xv; } break;
+                case LA_B1: V[LV_T * 64 + r] = t; V[LV_Y2 * 64 + r] = C > 1 ? g0 : V[LV_X * 64 + r]; break;
+                case LA_B2: V[LV_Y * 64 + r] = g0 - V[LV_T * 64 + r] - t; break;
+                default: {   // LA_ZN, LA_W: final values and the Chebyshev update d' = c_d d + c_z z (x += d')
+                    const double zv = o.act == LA_ZN ? t : g0 - t;
+                    if (o.act == LA_ZN) V[LV_ZN * 64 + r] = t;
+                    const size_t g = idx(o.k, r);
+                    double dn = a.c_z * zv;
+                    if (a.dold != nullptr && a.c_d != 0.0) dn = fma(a.c_d, a.dold[g], dn);
+                    a.dout[g] = dn;
+                    if (a.x != nullptr) a.x[g] += dn;
+                }
+            }
+        }
+        __syncthreads();   // the action's vectors are visible; the block's stage is free
+        if (tid == 0 && o.M != nullptr) issue_next();
+    }
+}
+
 }  // namespace mgk

@@ -139,6 +139,7 @@ struct mg_handle {
     double *frag_part = nullptr;  // TMA kernel: partial sums of rows that straddle two CTAs (sm_count x 36)
     int *frag_flag = nullptr;
     bool tma_ready = false;  // b == 36 and the kernel's shared-memory attribute is set
+    size_t line_smem_set = 0;  // dynamic shared memory line_apply_staged_kernel has been opted in for
     cudaStream_t stream = nullptr;      // active stream: the caller's, or cap_stream while a graph is captured
     cudaStream_t cap_stream = nullptr;  // internal non-default stream (the legacy default stream cannot capture)
     std::vector<Level> lev;
@@ -359,7 +360,7 @@ int launch_bsr(mg_handle *h, const Level &L, BsrArgs a, TmaExtra ex = TmaExtra{}
 #define BSR_CASE(B)                                                                                          \
     case B: {                                                                                                \
         int grid = (int)((L.n_brows + BsrCfg<B>::G - 1) / BsrCfg<B>::G);                                      \
-        if (B <= 12) grid = std::min(grid, h->sm_count * BsrCfg<B>::RESIDENT); /* resident grid, row groups in a loop */ \
+        if (B <= 12 && a.mode != MODE_PBJ) grid = std::min(grid, h->sm_count * BsrCfg<B>::RESIDENT); /* resident grid, row groups in a loop (not for the one-load-round PBJ apply: 15 % slower there) */ \
         LAUNCH(h, bsr_fused_kernel<B>, grid, BsrCfg<B>::THREADS, 0, a);                                       \
         break;                                                                                               \
     }
@@ -444,7 +445,16 @@ int line_apply(mg_handle *h, const Level &L, const double *rin, const double *do
     a.N = L.n_phi;
     a.b = h->b;
     a.done = nullptr;
-    LAUNCH(h, line_apply_kernel, (h->n_pol + LINE_WARPS - 1) / LINE_WARPS, LINE_WARPS * 32, 0, a);
+    const size_t smem = line_staged_smem(a.b, a.N);
+    if (a.b % 4 == 0 && smem <= 200 * 1024 && h->opt.kernel_variant == 0) {   // blocks staged through shared memory by bulk copies
+        if (smem > 48 * 1024 && smem > h->line_smem_set) {
+            CU(cudaFuncSetAttribute(line_apply_staged_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            h->line_smem_set = smem;
+        }
+        LAUNCH(h, line_apply_staged_kernel, h->n_pol, (4 * a.b + 31) / 32 * 32, smem, a);
+    } else {
+        LAUNCH(h, line_apply_kernel, (h->n_pol + LINE_WARPS - 1) / LINE_WARPS, LINE_WARPS * 32, 0, a);
+    }
     CU(cudaGetLastError());
     return MG_OK;
 }

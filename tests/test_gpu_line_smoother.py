@@ -30,9 +30,10 @@ def make(case, **opt):
     return w, H, s
 
 
+@pytest.mark.parametrize("variant", [0, 1])   # 0: blocks staged by bulk copies where b % 4 == 0; 1: one warp per line, per-lane row reads
 @pytest.mark.parametrize("case", list(CASES))
-def test_line_smoother_kernels_and_bounds(case):
-    w, H, s = make(case, coarse_mode=2)
+def test_line_smoother_kernels_and_bounds(case, variant):
+    w, H, s = make(case, coarse_mode=2, kernel_variant=variant)
     try:
         for l, L in enumerate(H.levels[:-1]):
             assert abs(s.get_level(l)["rho_est"] - L.rho_est) <= 1e-8 * L.rho_est      # power iteration with the line solve
