@@ -136,3 +136,36 @@ def test_c1_direct_coarse_solve(c1):
             assert np.abs(np.log10(np.array(info["hist"][:k]) / np.array(g["hist"][:k]))).max() <= 0.05
     finally:
         s.update_options(coarse_mode=1)
+
+
+@pytest.mark.slow
+def test_c3_fine_level_kernels_at_full_size():
+    """Config 3 "Large non-axisymmetric" at full size (8,000 nodes x 32 planes, b = 36: 256,000 block rows, 2,278,400 blocks,
+    23.6 GB of values: the value offsets pass 2^31) -- the fine-level kernels in the launch configuration bench.py times,
+    element by element against the oracle: SpMV, residual, PBJ apply, Chebyshev-PBJ smoothing from a zero and a non-zero
+    guess.  One level only (the oracle's 74 GB hierarchy does not fit the host): the Galerkin levels are covered at C1 size."""
+    import gc
+    w = small("C3", levels=1)
+    L = mg.Level(n_phi=w.n_phi, n_pol=w.n_pol, b=w.b, row_ptr=w.row_ptr, col_idx=w.col_idx, vals=w.vals)
+    L.dinv = mg.pbj_invert(L)
+    L.rho_est = mg.power_rho(L, 3)                 # any interval will do for a kernel comparison: 3 power steps
+    L.lam_min, L.lam_max = 0.1 * L.rho_est, 1.1 * L.rho_est
+    s = gpu_solver(w, eig_iters=3)
+    try:
+        assert abs(s.get_level(0)["rho_est"] - L.rho_est) <= 1e-9 * L.rho_est
+        s.set_cheb_bounds(0, L.lam_min, L.lam_max)
+        x = input_vector(L.n, w.seed, 11)
+        rhs = input_vector(L.n, w.seed, 12)
+        y_or = mg.spmv(L, x)
+        assert relmax(to_np(s.spmv(0, to_dev(x))), y_or) <= TOL_KERNEL
+        assert relmax(to_np(s.residual(0, to_dev(rhs), to_dev(x))), rhs - y_or) <= TOL_KERNEL
+        assert relmax(to_np(s.pbj_apply(0, to_dev(rhs))), mg.pbj_apply(L, rhs)) <= TOL_KERNEL
+        for nu, zero_guess in ((2, True), (2, False)):
+            x_or = mg.chebyshev(L, rhs, None if zero_guess else x, nu)
+            xg = to_dev(np.full(L.n, 7.0) if zero_guess else x)
+            s.smooth(0, to_dev(rhs), xg, nu, zero_guess)
+            assert relmax(to_np(xg), x_or) <= TOL_KERNEL
+    finally:
+        s.destroy()
+        del w, L
+        gc.collect()
