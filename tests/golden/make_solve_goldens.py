@@ -42,6 +42,7 @@ CASES = {
     # config 2 at full size (16 planes) with the direct coarsest-level solve
     "C2-16_direct": ("C2-16", {}, dict(coarse_mode=2)),
     "C2-32_direct": ("C2-32", {}, dict(coarse_mode=2)),
+    "C2-64_direct": ("C2-64", {}, dict(coarse_mode=2)),
     # config 3's recipe (non-axisymmetric, beta = 0.5, sigma = 1e-4, delta = 0.15, 32 -> 2 planes) on a reduced mesh
     "C3r_default": ("C3", dict(mesh=(4, 16)), dict(coarse_mode=0)),
     "C3r_direct": ("C3", dict(mesh=(4, 16)), dict(coarse_mode=2)),

@@ -21,7 +21,7 @@ from gpu_util import gpu_solver, to_dev, to_np
 pytestmark = [pytest.mark.gpu, pytest.mark.slow]
 
 GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
-CASES = ["C0_direct", "C0_default", "C2r_direct", "C2r_default", "C3r_direct", "C3r_default", "C1_direct", "C2-16_direct", "C2-32_direct",
+CASES = ["C0_direct", "C0_default", "C2r_direct", "C2r_default", "C3r_direct", "C3r_default", "C1_direct", "C2-16_direct", "C2-32_direct", "C2-64_direct",
          "C1_default_2its"]
 
 
