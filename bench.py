@@ -210,6 +210,18 @@ class OracleUnits:
             t0 = time.perf_counter()
             mg.chebyshev(L0, w.rhs, None, 1)
             out["chebyshev_sweep_fine_s"] = time.perf_counter() - t0
+            # the single-thread figure of the fine-level SpMV: OpenMP threads of the oracle's C loops set to 1
+            try:
+                import ctypes
+                omp = ctypes.CDLL("libgomp.so.1")
+                nthr = omp.omp_get_max_threads()
+                omp.omp_set_num_threads(1)
+                t0 = time.perf_counter()
+                mg.spmv(L0, w.rhs)
+                out["spmv_fine_1_thread_s"] = time.perf_counter() - t0
+                omp.omp_set_num_threads(nthr)
+            except OSError:
+                pass
             H.opt.coarse_fixed_sweeps = 8
             t0 = time.perf_counter()
             mg.vcycle(H, w.rhs)
