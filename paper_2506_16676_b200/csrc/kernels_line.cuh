@@ -382,11 +382,14 @@ __global__ void __launch_bounds__(LINE_WARPS * 32) line_apply_kernel(const LineA
 // The same recurrences as line_apply_kernel, as a list of 5 (N - 1) mat-vec OPERATIONS per node executed by one CTA:
 // thread t owns the b/4-element segment t % 4 of row t / 4 of every block (the mapping of the b = 36 TMA kernel: the four
 // partial sums of a row meet by two shuffles).  The blocks an apply reads are STATIC, so thread 0 walks the operation list
-// ahead of the arithmetic with 1-D bulk async copies (TMA engine, SASS UBLKCP) into a ring of LS_STAGES block buffers: the
+// ahead of the arithmetic with 1-D bulk async copies (TMA engine, SASS UBLKCP) into a small ring of LS_STAGES block buffers: the
 // block of an operation is in shared memory before the operation starts, and every global read of a block is one coalesced
 // copy.  (line_apply_kernel walks the same ~5N dependent mat-vecs with per-lane row reads: 32 different lines per load
 // instruction, 2.5 TB/s on C1's level 0.)
-constexpr int LS_STAGES = 3;
+#ifndef MG_LS_STAGES
+#define MG_LS_STAGES 2   /* measured on C1 level 0: 2 stages 249 us, 3: 285, 4: 293, 6: 325 (more CTAs per SM beat a deeper ring) */
+#endif
+constexpr int LS_STAGES = MG_LS_STAGES;
 enum { LA_Q = 0, LA_Y, LA_T, LA_X, LA_B1, LA_B2, LA_ZN, LA_W };           // what the writer lanes do with the result t
 enum { LV_Y = 0, LV_Q, LV_X, LV_T, LV_Y2, LV_ZN, LV_COUNT };               // vectors in shared memory (64 doubles each)
 struct LineOp {

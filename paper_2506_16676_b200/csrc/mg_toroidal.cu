@@ -2108,6 +2108,6 @@ int mg_debug_ds_stamps(unsigned long long *host, int n) {
 }
 #endif
 
-const char *mg_version(void) { return "mg_toroidal 0.1.0 (sm_100a)"; }
+const char *mg_version(void) { return "mg_toroidal 0.2.0 (sm_100a)"; }
 
 }  // extern "C"

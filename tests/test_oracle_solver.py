@@ -277,3 +277,28 @@ def test_direct_coarse_mode_is_the_exact_coarse_solve():
     assert np.abs(mg.vcycle(H, r) - M @ r).max() <= 1e-10 * np.abs(M @ r).max()
     x, it, conv, hist = mg.solve(H, w.rhs, 1e-8)
     assert conv and np.linalg.norm(w.rhs - mats[0][0] @ x) <= 1.05e-8 * np.linalg.norm(w.rhs)
+
+
+@pytest.mark.slow
+def test_solve_against_dense_lu_at_full_config_0_size():
+    """brute force at FULL config-0 size (27,648 unknowns, b = 36): the oracle's complete solve (V-cycle
+    preconditioned FGMRES to rtol 1e-8) against LAPACK's dense LU of the assembled matrix.  With r = b - A x,
+    ||x - x*|| <= ||A^-1|| ||r|| <= kappa * rtol * ||x*||; kappa_2 <= sqrt(kappa_1 kappa_inf), both from LAPACK's dgecon."""
+    import scipy.linalg as sla
+    w = make_workload("C0")
+    H = hierarchy(w, coarse_mode=2)                      # the coarsest level by sparse LU: the cycle is a fixed operator
+    x, it, conv, hist = mg.solve(H, w.rhs, 1e-8)
+    assert conv and hist[-1] <= 1e-8
+    A = mg.to_dense(H.levels[0])
+    anorm1, anormi = np.abs(A).sum(axis=0).max(), np.abs(A).sum(axis=1).max()
+    lu, piv = sla.lu_factor(A, overwrite_a=True, check_finite=False)
+    xstar = sla.lu_solve((lu, piv), w.rhs, check_finite=False)
+    rc1, _ = sla.lapack.dgecon(lu, anorm1, norm="1")
+    rci, _ = sla.lapack.dgecon(lu, anormi, norm="I")
+    kappa2_bound = float(np.sqrt(1.0 / rc1 / rci))
+    err = np.linalg.norm(x - xstar) / np.linalg.norm(xstar)
+    assert err <= kappa2_bound * 1e-8
+    assert err <= 1e-4                                    # and it is a solution in the plain sense (kappa ~ 1e4 here)
+    true_rel = np.linalg.norm(w.rhs - mg.spmv(H.levels[0], x)) / np.linalg.norm(w.rhs)
+    assert true_rel <= 1.01e-8 and abs(hist[-1] - true_rel) <= 1e-3 * true_rel   # the Arnoldi estimate IS the residual
+    assert it == 91                                       # tests/golden/solve_C0_direct.json
