@@ -520,6 +520,9 @@ __device__ __forceinline__ void ds_st(double *p, const double v) {
     asm volatile("st.relaxed.gpu.global.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory");
 }
 __device__ __forceinline__ bool ds_missing(const double v) { return __double_as_longlong(v) == -1ll; }
+// A poll gives up after this many tries (a fraction of a second): a right-hand side that itself holds the sentinel bit pattern (a NaN with an
+// all-ones payload) must end in NaNs, not in a hang.
+constexpr int DS_SPIN_MAX = 1 << 18;   // (a legitimate wait is a few hundred polls)
 
 // One CTA's share of one step: per job the rows [ra, rb) of the level set.  Stream order: the packed off-diagonal rows of
 // job 0 (`rps` rows per stage), those of job 1, then the rows of S^-1 of job 0 in segments of DS_SEG doubles, then job 1's.
@@ -713,6 +716,7 @@ __global__ void __launch_bounds__(DS_THREADS, 1) direct_solve_persistent_kernel(
                             xv[w][v] = (w < ne && ncol[w] >= 0 && cx < b) ? ds_ld(src + (size_t)ncol[w] * b + cx) : 0.0;
                         }
                     bool again;
+                    int spins = 0;
                     do {
                         again = false;
 #pragma unroll
@@ -723,7 +727,7 @@ __global__ void __launch_bounds__(DS_THREADS, 1) direct_solve_persistent_kernel(
                                     xv[w][v] = ds_ld(src + (size_t)ncol[w] * b + sub + v * DS_TPR);
                                     again = again || ds_missing(xv[w][v]);
                                 }
-                    } while (again);
+                    } while (again && ++spins < DS_SPIN_MAX);
                     const int ql = row - P.ra;                       // row within the piece
                     const long long cc = cnt + (pi ? d.p[0].nA : 0) + ql / P.rps;
                     const int st = (int)(cc % ST);
@@ -745,7 +749,7 @@ __global__ void __launch_bounds__(DS_THREADS, 1) direct_solve_persistent_kernel(
                             for (int cx = sub; cx < b; cx += DS_TPR) {
                                 double x1;
                                 do x1 = ds_ld(src + (size_t)col * b + cx);
-                                while (ds_missing(x1));
+                                while (ds_missing(x1) && ++spins < DS_SPIN_MAX);
                                 acc = fma(As[w * b + cx], x1, acc);
                             }
                     }
@@ -782,6 +786,7 @@ __global__ void __launch_bounds__(DS_THREADS, 1) direct_solve_persistent_kernel(
                     tv[u] = i < tlen ? ds_ld(a.tb + d.t0 + tbase + i) : 0.0;
                 }
                 bool again;
+                int spins = 0;
                 do {
                     again = false;
 #pragma unroll
@@ -790,7 +795,7 @@ __global__ void __launch_bounds__(DS_THREADS, 1) direct_solve_persistent_kernel(
                             tv[u] = ds_ld(a.tb + d.t0 + tbase + i0 + tid + u * DS_WARPS * 32);
                             again = again || ds_missing(tv[u]);
                         }
-                } while (again);
+                } while (again && ++spins < DS_SPIN_MAX);
 #pragma unroll
                 for (int u = 0; u < 16; ++u) {
                     const int i = i0 + tid + u * DS_WARPS * 32;
@@ -843,9 +848,10 @@ __global__ void __launch_bounds__(DS_THREADS, 1) direct_solve_persistent_kernel(
                         ds_st(a.yb + gi, sum);
                         if (P.final) ds_st(a.xb + gi, sum);   // the middle level set: its result is also the first x
                     } else {
+                        int spins = 0;
                         double yk;                            // y_k of the elimination phase (written many steps ago, possibly
                         do yk = ds_ld(a.yb + gi);             // by another CTA: the steps pair the level sets differently)
-                        while (ds_missing(yk));
+                        while (ds_missing(yk) && ++spins < DS_SPIN_MAX);
                         sum = yk - sum;
                         ds_st(a.xb + gi, sum);
                     }

@@ -68,3 +68,27 @@ def test_solve_with_direct_coarse_level(case):
         assert true_rel <= 1.05e-8 and info["coarse_iters_total"] == 0
     finally:
         s.destroy()
+
+
+def test_sentinel_bit_pattern_in_the_right_hand_side_does_not_hang():
+    """The persistent kernel exchanges vectors through buffers pre-filled with a sentinel (a NaN with an all-ones payload) that
+    readers poll.  A right-hand side that itself holds that bit pattern must come back as NaNs in bounded time, not hang."""
+    import time
+    import torch
+    w, H, s = make("b36-3lev")
+    try:
+        Lc = H.levels[-1]
+        rc = to_dev(input_vector(Lc.n, w.seed, 63))
+        e, _ = s.coarse_solve(rc)                       # builds the factorisation; a normal solve first
+        assert s.direct_info()["persistent"]
+        bad = rc.clone()
+        bad.view(torch.int64)[5] = -1                   # 0xFFFFFFFFFFFFFFFF
+        t0 = time.perf_counter()
+        e_bad, _ = s.coarse_solve(bad)
+        torch.cuda.synchronize()
+        assert time.perf_counter() - t0 < 120.0
+        assert bool(torch.isnan(e_bad).any())
+        e2, _ = s.coarse_solve(rc)                      # and the next solve is clean again (the buffers are re-filled per launch)
+        assert np.array_equal(to_np(e2), to_np(e))
+    finally:
+        s.destroy()
