@@ -50,6 +50,10 @@ CASES = {
     # GMRES steps of 0.56 GB each: days of CPU time): the residual history of the first iterations and the oracle's
     # coarsest-level iteration count per V-cycle, which bench.py's cpu_baseline estimate uses
     "C1_default_2its": ("C1", {}, dict(coarse_mode=0, maxit=2)),
+    # NEXT-4 at config size: the toroidal-line block-Jacobi smoother with the direct coarsest-level solve
+    "C0_direct_line": ("C0", {}, dict(coarse_mode=2, smoother=2)),
+    "C2-16_direct_line": ("C2-16", {}, dict(coarse_mode=2, smoother=2)),
+    "C1_direct_line": ("C1", {}, dict(coarse_mode=2, smoother=2)),
 }
 
 

@@ -8,6 +8,7 @@ tolerance at different steps, a wrong one leaves the band.
 * ``*_direct``: coarse_mode = 2 on both sides (oracle: sparse LU; library: block-tridiagonal Schur inverses) -- the
   cycle is a fixed linear operator, histories agree to many digits.
 * ``*_default``: the configs' PBJ-GMRES(100) coarse solve to 1e-10 on both sides (an adaptive inner solve).
+* ``*_line``: the toroidal-line block-Jacobi smoother (smoother = 2) on both sides.
 """
 import json
 import os
@@ -22,7 +23,7 @@ pytestmark = [pytest.mark.gpu, pytest.mark.slow]
 
 GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
 CASES = ["C0_direct", "C0_default", "C2r_direct", "C2r_default", "C3r_direct", "C3r_default", "C1_direct", "C2-16_direct", "C2-32_direct", "C2-64_direct",
-         "C1_default_2its"]
+         "C1_default_2its", "C0_direct_line", "C2-16_direct_line", "C1_direct_line"]
 
 
 def load(case):
@@ -43,7 +44,7 @@ def test_solve_matches_oracle_golden(case):
     o = g["options"]
     s = gpu_solver(w, coarse_mode=o["coarse_mode"], nu_pre=o["nu_pre"], nu_post=o["nu_post"], restart=o["restart"],
                    maxit=o["maxit"], coarse_rtol=o["coarse_rtol"], coarse_restart=o["coarse_restart"],
-                   coarse_maxit=o["coarse_maxit"])
+                   coarse_maxit=o["coarse_maxit"], smoother=o.get("smoother", 0))
     try:
         for l, rho in enumerate(g["rho_est"]):           # the oracle's Chebyshev intervals (the library's own agree to 1e-9)
             assert abs(s.get_level(l)["rho_est"] - rho) <= 1e-8 * rho
