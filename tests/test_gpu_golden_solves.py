@@ -8,6 +8,8 @@ tolerance at different steps, a wrong one leaves the band.
 * ``*_direct``: coarse_mode = 2 on both sides (oracle: sparse LU; library: block-tridiagonal Schur inverses) -- the
   cycle is a fixed linear operator, histories agree to many digits.
 * ``*_default``: the configs' PBJ-GMRES(100) coarse solve to 1e-10 on both sides (an adaptive inner solve).
+* ``*_gmres11``: the paper's own level smoother, one PBJ-preconditioned GMRES iteration before and after (smoother = 1,
+  V(1,1)): a NONLINEAR cycle, held to the same bands.
 * ``*_line``: the toroidal-line block-Jacobi smoother (smoother = 2) on both sides.
 """
 import json
@@ -23,7 +25,8 @@ pytestmark = [pytest.mark.gpu, pytest.mark.slow]
 
 GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
 CASES = ["C0_direct", "C0_default", "C2r_direct", "C2r_default", "C3r_direct", "C3r_default", "C1_direct", "C2-16_direct", "C2-32_direct", "C2-64_direct",
-         "C1_default_2its", "C0_direct_line", "C2-16_direct_line", "C1_direct_line"]
+         "C1_default_2its", "C0_direct_line", "C2-16_direct_line", "C1_direct_line",
+         "C0_direct_gmres11", "C1_direct_gmres11"]
 
 
 def load(case):
