@@ -119,7 +119,8 @@ struct GmresDev {
     double *hnext;     // h_{j+1,j} (or beta): divisor for the next basis vector
     double *tol;       // absolute tolerance rtol*||rhs||
     double *hist;      // hist[it] = residual estimate (absolute), it = 0..maxit
-    int *status;       // [0] done, [1] j_used, [2] it, [3] converged
+    int *status;       // [0] done, [1] j_used, [2] it, [3] converged, [4] done as the latest Gram-Schmidt kernel saw it (the flag a
+                       //     SpMV running BESIDE the deferred Givens update reads: nothing writes it while that SpMV runs)
     int m, maxit;
 };
 
@@ -158,7 +159,8 @@ __device__ __forceinline__ void gmres_update_dev(const GmresDev &s, const int j)
 // coefficients are fetched with coalesced independent loads and the rotation recurrence runs out of shared memory.  (The
 // one-thread version above walks ~4 j dependent global loads: ~13 us at j = 50, a third of the whole Gram-Schmidt kernel.)
 // Same arithmetic in the same order, so the results are bit-identical.
-__device__ __forceinline__ void gmres_update_warp(const GmresDev &s, const int j, const int lane, double *sc, double *scs, double *ssn) {
+__device__ __forceinline__ void gmres_update_warp(const GmresDev &s, const int j, const int lane, double *sc, double *scs, double *ssn,
+                                                  const bool write_hnext = true) {
     if (s.status[0] != 0) return;   // (uniform: every lane reads the same value)
     for (int i = lane; i <= j; i += 32) {
         sc[i] = __ldcg(s.h1 + i) + __ldcg(s.h2 + i);
@@ -171,7 +173,7 @@ __device__ __forceinline__ void gmres_update_warp(const GmresDev &s, const int j
     if (lane == 0) {
         const double hn = sqrt(fmax(*s.nrm2, 0.0));
         sc[j + 1] = hn;
-        *s.hnext = hn;
+        if (write_hnext) *s.hnext = hn;
         for (int i = 0; i < j; ++i) {
             const double t = scs[i] * sc[i] + ssn[i] * sc[i + 1];
             sc[i + 1] = -ssn[i] * sc[i] + scs[i] * sc[i + 1];
@@ -295,6 +297,8 @@ struct OrthArgs {
     int slice;             // elements per CTA, even
     int cap;               // basis vectors cached in shared memory
     int ld;                // >= m + 1
+    int defer_update;      // 1: the last CTA writes ||w||^2 and h_{j+1,j} only; the Hessenberg / Givens / stop-test update of
+                           // column j runs in gmres_givens_kernel, beside the next SpMV (coarsest-level cycle)
     double eta2;           // selective reorthogonalisation (Daniel-Gragg-Kaufman-Stewart): the second pass is skipped
                            // when ||w - V h1||^2 >= eta2 ||w||^2, estimated as ||w||^2 - |h1|^2; 0 = always two passes
 };
@@ -346,7 +350,10 @@ __device__ __forceinline__ double orth_dot_range(const double2 *__restrict__ src
 __global__ void __launch_bounds__(ORTH_THREADS, 1) gmres_orth_fused_kernel(const OrthArgs a) {
     namespace cg = cooperative_groups;
     cg::grid_group grid = cg::this_grid();
-    if (a.done != nullptr && *a.done != 0) return;   // written by an earlier kernel: every CTA takes the same branch
+    if (a.done != nullptr && *a.done != 0) {   // written by an earlier kernel: every CTA takes the same branch
+        if (a.defer_update && blockIdx.x == 0 && threadIdx.x == 0) a.dev.status[4] = 1;
+        return;
+    }
     extern __shared__ __align__(16) double orth_sm[];
     double *ws = orth_sm;                 // [slice]   this CTA's slice of w
     double *hs = ws + a.slice;            // [ld]      coefficients of the current pass
@@ -518,11 +525,23 @@ __global__ void __launch_bounds__(ORTH_THREADS, 1) gmres_orth_fused_kernel(const
         if (lane == 0) {
             *a.dev.nrm2 = t;
             *a.counter = 0;
+            if (a.defer_update) *a.dev.hnext = sqrt(fmax(t, 0.0));
         }
         __syncwarp();
-        gmres_update_warp(a.dev, a.j, lane, hd, hd + a.ld, hs);   // hd [2 ld] and hs [ld] are free by now (ld >= m + 2)
+        if (!a.defer_update)
+            gmres_update_warp(a.dev, a.j, lane, hd, hd + a.ld, hs);   // hd [2 ld] and hs [ld] are free by now (ld >= m + 2)
     }
     MG_ORTH_STAMP(10);
+}
+
+// The deferred update of column j (OrthArgs::defer_update): one warp, launched on a side branch of the captured coarsest-level
+// cycle, so that the serial rotation recurrence and the stop test run BESIDE the next SpMV -- which needs h_{j+1,j} and the new
+// vector but nothing of the Givens state -- instead of in front of it.  That SpMV reads status[4], the `done` flag as the
+// Gram-Schmidt kernel before it saw it (nothing writes it while the SpMV runs): after convergence it computes ONE vector nobody
+// uses (the basis slot it writes is not part of the solution update).  The next Gram-Schmidt kernel is ordered after both.
+__global__ void __launch_bounds__(32) gmres_givens_kernel(const GmresDev dev, const int j, const int ld) {
+    extern __shared__ double givens_sm[];   // 3 ld doubles, ld >= m + 1
+    gmres_update_warp(dev, j, (int)threadIdx.x, givens_sm, givens_sm + ld, givens_sm + 2 * ld, false);
 }
 
 // dst = src / *denom   (v_{j+1} = w / h_{j+1,j}); dst may equal src.
@@ -551,7 +570,7 @@ __global__ void __launch_bounds__(256) hashed_start_kernel(double *__restrict__ 
 
 __global__ void gmres_set_tol_kernel(GmresDev s, const double rtol) {
     *s.tol = rtol * sqrt(fmax(*s.nrm2, 0.0));
-    s.status[0] = 0; s.status[1] = 0; s.status[2] = 0; s.status[3] = 0;
+    s.status[0] = 0; s.status[1] = 0; s.status[2] = 0; s.status[3] = 0; s.status[4] = 0;
 }
 
 // Cycle begin: beta = ||r||; converged if beta <= tol; g = beta e_1.
