@@ -1344,6 +1344,7 @@ int coarse_solve_internal(mg_handle *h) {
         CU(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
         h->stream = h->cap_stream;
         h->capturing = true;
+        h->join_pending = false;   // (a failed earlier attempt may have left its side branch open)
         h->capture_count = 0;
         std::memset(h->graph_hist, 0, sizeof(h->graph_hist));
         const int rc = coarse_cycle_enqueue(h);
