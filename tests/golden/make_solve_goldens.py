@@ -54,7 +54,6 @@ CASES = {
     "C0_direct_line": ("C0", {}, dict(coarse_mode=2, smoother=2)),
     "C2-16_direct_line": ("C2-16", {}, dict(coarse_mode=2, smoother=2)),
     "C1_direct_line": ("C1", {}, dict(coarse_mode=2, smoother=2)),
-    "C2-32_direct_line": ("C2-32", {}, dict(coarse_mode=2, smoother=2)),
     # NEXT-1 at config size: the paper's level smoother, nu iterations of PBJ-preconditioned GMRES, V(1,1)
     "C0_direct_gmres11": ("C0", {}, dict(coarse_mode=2, smoother=1, nu_pre=1, nu_post=1)),
     "C1_direct_gmres11": ("C1", {}, dict(coarse_mode=2, smoother=1, nu_pre=1, nu_post=1)),

@@ -27,7 +27,7 @@ GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
 CASES = ["C0_direct", "C0_default", "C2r_direct", "C2r_default", "C3r_direct", "C3r_default", "C1_direct", "C2-16_direct", "C2-32_direct", "C2-64_direct",
          "C1_default_2its", "C0_direct_line", "C2-16_direct_line", "C1_direct_line",
          "C0_direct_gmres11", "C1_direct_gmres11", "C1_direct_gmres66", "C1_direct_5lev",
-         "C2-32_direct_line", "C2-16_direct_gmres11"]
+         "C2-16_direct_gmres11"]
 
 
 def load(case):
