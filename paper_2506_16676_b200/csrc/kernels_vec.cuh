@@ -586,15 +586,59 @@ __global__ void gmres_begin_kernel(GmresDev s) {
 }
 
 // Back substitution H y = g over the j_used columns of this cycle.  One warp: the inner sum over l > i is split
-// across the lanes (fixed lane -> l mapping and shuffle tree: deterministic).
+// across the lanes (fixed lane -> l mapping and shuffle tree: deterministic).  Fast path (j_used <= 256): y lives in shared
+// memory and the entries of row i-1 (which do not depend on y) are loaded while row i is reduced, so a row costs a shuffle
+// tree and a division instead of two dependent global round trips (100 columns: ~150 -> ~35 us per restart cycle).  Same
+// operations in the same order as the plain loop below: bit-identical y.
 __global__ void __launch_bounds__(32) gmres_solve_y_kernel(GmresDev s) {
     const int ju = s.status[1];
     const int lane = threadIdx.x;
+    constexpr int NL = 8;
+    __shared__ double ys[32 * NL];
+    const size_t ld = (size_t)s.m + 1;
+    if (ju <= 32 * NL) {
+        double hn[NL], gn = 0.0, dn = 1.0;
+        {
+            const int i = ju - 1;   // row ju-1 has no entries right of the diagonal
+#pragma unroll
+            for (int k = 0; k < NL; ++k) hn[k] = 0.0;
+            if (lane == 0 && i >= 0) { gn = s.g[i]; dn = s.H[(size_t)i * ld + i]; }
+        }
+        for (int i = ju - 1; i >= 0; --i) {
+            double hc[NL];
+#pragma unroll
+            for (int k = 0; k < NL; ++k) hc[k] = hn[k];
+            const double gc = gn, dc = dn;
+            if (i > 0) {
+                const int ip = i - 1;
+#pragma unroll
+                for (int k = 0; k < NL; ++k) {
+                    const int l = ip + 1 + lane + 32 * k;
+                    hn[k] = (l < ju) ? s.H[(size_t)l * ld + ip] : 0.0;
+                }
+                if (lane == 0) { gn = s.g[ip]; dn = s.H[(size_t)ip * ld + ip]; }
+            }
+            double t = 0.0;
+#pragma unroll
+            for (int k = 0; k < NL; ++k) {
+                const int l = i + 1 + lane + 32 * k;
+                if (l < ju) t = fma(hc[k], ys[l], t);
+            }
+            t = warp_sum(t);
+            if (lane == 0) {
+                const double yi = (gc - t) / dc;
+                ys[i] = yi;
+                s.y[i] = yi;
+            }
+            __syncwarp();
+        }
+        return;
+    }
     for (int i = ju - 1; i >= 0; --i) {
         double t = 0.0;
-        for (int l = i + 1 + lane; l < ju; l += 32) t = fma(s.H[(size_t)l * (s.m + 1) + i], s.y[l], t);
+        for (int l = i + 1 + lane; l < ju; l += 32) t = fma(s.H[(size_t)l * ld + i], s.y[l], t);
         t = warp_sum(t);
-        if (lane == 0) s.y[i] = (s.g[i] - t) / s.H[(size_t)i * (s.m + 1) + i];
+        if (lane == 0) s.y[i] = (s.g[i] - t) / s.H[(size_t)i * ld + i];
         __syncwarp();
     }
 }
